@@ -1,0 +1,121 @@
+/*
+ * dks_poisson.h -- C ABI of the B200-native open-boundary FFT Poisson solver.
+ *
+ * The operation (arXiv:1509.07685, "The Dynamical Kernel Scheduler - Part 1"):
+ *   PAPER.md:119-122, section 3.1.1, Eq. (2):
+ *       phi[i,j,k] = hx*hy*hz * sum_{i',j',k'} rho[i',j',k'] * G((i-i')hx, (j-j')hy, (k-k')hz)
+ *   computed as (section 3.1.1)
+ *       phi = hx*hy*hz * FT^-1{ FT{rho} (x) FT{G} }
+ *   on Hockney's doubled grid 2Mx x 2My x 2Mz (section 3.1), with
+ *       G(u,v,w) = 1 / (4*pi*eps0*sqrt(u^2+v^2+w^2))        (the 1/(4 pi eps0) follows
+ *   from the PDE laplace(phi) = -rho/eps0 at PAPER.md:104; eps0 = 8.8541878128e-12 F/m).
+ *   The paper's GPU implementation (section 3.1.2) has "separate kernels to calculate
+ *   the Greens function and perform the multiplication" around a library FFT; here every step is a
+ *   hand-written sm_100a kernel and padding, multiplication, cropping and scaling are fused into
+ *   the FFT passes.
+ *
+ * Conventions
+ *   - mesh n = (nx, ny, nz) = the paper's (Mx, My, Mz); every n must be a power of two in [8, 1024]
+ *     (Table 1, uses powers of two only).
+ *   - rho, phi: DEVICE pointers, contiguous fp64, x fastest: linear index (k*ny + j)*nx + i, i.e. a
+ *     [nz][ny][nx] array; 16-byte aligned.  phi in volts for rho in C/m^3 and h in metres.
+ *   - G(0,0,0) defaults to G at r0 = min(hx,hy,hz)/2 (the paper is silent; reading A2).
+ *   - All calls return DKS_OK (0) or a negative dks_status; nothing throws or aborts across the ABI.
+ *     dks_last_error() returns a thread-local, NUL-terminated message for the last failure.
+ *   - A plan is a host object owning host metadata and device twiddle tables.  It is not re-entrant:
+ *     one solve in flight per plan.
+ *   - There is no CPU fallback.  Without a compute-capability 10.x device every compute entry point
+ *     returns DKS_ERR_UNSUPPORTED_DEVICE / DKS_ERR_CUDA.
+ */
+#ifndef DKS_POISSON_H
+#define DKS_POISSON_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum dks_status {
+    DKS_OK = 0,
+    DKS_ERR_INVALID_ARG = -1,        /* NULL pointer, n not a power of two in [8,1024], h <= 0 or not finite */
+    DKS_ERR_UNSUPPORTED_DEVICE = -2, /* current device is not compute capability 10.x                      */
+    DKS_ERR_NO_WORKSPACE = -3,       /* (reserved)                                                         */
+    DKS_ERR_WORKSPACE_TOO_SMALL = -4,/* dks_poisson_set_workspace: bytes < dks_poisson_workspace_bytes     */
+    DKS_ERR_NOT_SETUP = -5,          /* dks_poisson_solve before dks_greens_setup (or after a spacing change) */
+    DKS_ERR_CUDA = -6                /* a CUDA runtime call failed; see dks_last_error()                   */
+} dks_status;
+
+typedef struct dks_poisson_plan dks_poisson_plan;   /* opaque */
+
+/* Creates a plan for an nx x ny x nz mesh with spacings hx, hy, hz [m].  Host-only: validates the
+ * arguments and computes the twiddle tables on the host; touches no device.  Returns NULL on
+ * failure (dks_last_error() says why). */
+dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, double hx, double hy, double hz);
+
+/* Frees the plan, its device tables and (if plan-owned) its workspace.  NULL is allowed. */
+void dks_poisson_plan_destroy(dks_poisson_plan *plan);
+
+/* Step a0 ("separate kernels to calculate the Greens function"):
+ * builds G on the octant of the doubled grid (mirror rule i' = min(i, 2n-i)), transforms it
+ * (the transform of the even extension is real and even, so only the (nx+1)(ny+1)(nz+1) octant is
+ * kept) and folds the factor hx*hy*hz/(8 nx ny nz) in.  Allocates the plan-owned workspace on first
+ * use if none was attached.  Asynchronous on the plan's setup stream (default: the legacy default
+ * stream); a later dks_poisson_solve on another stream is ordered after it by an event. */
+int dks_greens_setup(dks_poisson_plan *plan);
+
+/* The hot path: phi = hx hy hz FT^-1{FT{rho} (x) FT{G}} cropped to the mesh.
+ * rho_dev, phi_dev: device pointers as described above; rho_dev is only read; phi_dev may alias
+ * rho_dev.  stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous and stream-ordered:
+ * no host synchronisation, no allocation; CUDA-graph capturable.  Five kernel launches. */
+int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, void *stream);
+
+/* Same solve with HOST buffers (the end-to-end path of the paper: rho is copied to
+ * the device and phi back every step).  rho_host/phi_host: host pointers ([nz][ny][nx] fp64; pinned
+ * memory recommended).  Copies H2D, solves, copies D2H on `stream`, then synchronises the stream.
+ * The staging buffer is part of the workspace. */
+int dks_poisson_solve_host(dks_poisson_plan *plan, const double *rho_host, double *phi_host, void *stream);
+
+/* Changes the mesh spacings (they are time dependent).  Invalidates the Green's
+ * transform: call dks_greens_setup again before the next solve. */
+int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double hz);
+
+/* Overrides G(0,0,0); NaN restores the default rule.  Invalidates the Green's transform. */
+int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
+
+/* Bytes of device workspace the plan needs (buffers A, B, the Green's octant, the host-path staging
+ * buffer). */
+size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
+
+/* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace; 256-byte aligned,
+ * at least dks_poisson_workspace_bytes().  The caller keeps ownership and must keep it alive.
+ * Invalidates the Green's transform. */
+int dks_poisson_set_workspace(dks_poisson_plan *plan, void *dev_ptr, size_t bytes);
+
+/* Stream used by dks_greens_setup (default NULL = legacy default stream). */
+int dks_poisson_set_stream(dks_poisson_plan *plan, void *stream);
+
+/* Per-pass timing.  slots > 0: dks_poisson_solve records CUDA events on its stream around each of
+ * its five passes (still asynchronous) and keeps those of the last `slots` solves (slots <= 1024);
+ * slots = 0 switches it off.  dks_poisson_pass_times waits for the recorded solves and writes up to
+ * `count` durations in milliseconds (pass order P1..P5), each the mean over the recorded solves;
+ * returns the number of passes written or a negative status. */
+int dks_poisson_set_profiling(dks_poisson_plan *plan, int slots);
+int dks_poisson_pass_times(dks_poisson_plan *plan, float *ms_out, int count);
+
+/* Facts about the plan, for benchmarks and tests. */
+int    dks_poisson_launches_per_solve(const dks_poisson_plan *plan);   /* kernels launched by one solve   */
+double dks_poisson_model_bytes(const dks_poisson_plan *plan, int pass); /* algorithmic HBM bytes of pass 1..5; pass 0 = whole solve (DESIGN.md model M3) */
+const char *dks_poisson_pass_name(const dks_poisson_plan *plan, int pass); /* kernel variant used for pass 1..5 */
+
+/* Copies the Green's octant (real, [(nz+1)][(ny+1)][(nx+1)], scale folded in) to a host buffer of
+ * (nx+1)(ny+1)(nz+1) doubles; synchronises.  For tests. */
+int dks_poisson_copy_greens_hat(dks_poisson_plan *plan, double *host_out);
+
+/* Thread-local message describing the last error in this thread ("" if none). */
+const char *dks_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DKS_POISSON_H */

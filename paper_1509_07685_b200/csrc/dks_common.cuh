@@ -1,0 +1,45 @@
+// Shared device helpers for the dks_poisson kernels (sm_100a).  fp64 complex arithmetic on double2.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace dks {
+
+typedef double2 cplx;   // .x = re, .y = im
+
+__device__ __forceinline__ cplx cmake(double re, double im) { return make_double2(re, im); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+// a * b
+__device__ __forceinline__ cplx cmul(cplx a, cplx b)
+{
+    return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+// a * conj(b)
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b)
+{
+    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -(a.x * b.y)));
+}
+// a * (-i)  and  a * (+i)
+__device__ __forceinline__ cplx cmul_mi(cplx a) { return make_double2(a.y, -a.x); }
+__device__ __forceinline__ cplx cmul_pi(cplx a) { return make_double2(-a.y, a.x); }
+
+// bit reversal of the low `bits` bits
+__device__ __forceinline__ int brev(int v, int bits) { return (int)(__brev((unsigned)v) >> (32 - bits)); }
+
+// 128-bit global access with streaming hints: every byte of the intermediate buffers is touched once
+// per pass, so do not allocate in L1.
+__device__ __forceinline__ cplx ldg_stream(const cplx *p)
+{
+    cplx r;
+    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void stg_stream(cplx *p, cplx v)
+{
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+
+}  // namespace dks

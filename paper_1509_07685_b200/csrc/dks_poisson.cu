@@ -1,0 +1,433 @@
+// dks_poisson.cu -- plan / workspace / stream management and the C ABI (include/dks_poisson.h).
+//
+// The plan owns: host metadata, device twiddle tables, profiling events, an ordering event between
+// dks_greens_setup and dks_poisson_solve, and (unless the caller attached one) the device workspace
+//     [ A | B | Ghat octant | host-path staging ].
+// dks_poisson_solve launches five kernels on the caller's stream and returns; it neither allocates
+// nor synchronises ("streams for asynchronous copy/compute").
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/dks_poisson.h"
+#include "dks_passes_generic.cuh"
+
+using namespace dks;
+
+// ------------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define DKS_CUDA(call)                                                                            \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(DKS_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),     \
+                        __FILE__, __LINE__);                                                      \
+    } while (0)
+
+extern "C" const char *dks_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------------------------------------
+// plan
+// ------------------------------------------------------------------------------------------------
+struct dks_poisson_plan {
+    MeshDims d;
+    double hx, hy, hz;
+    double g0_override;                 // NaN = default rule
+    // device
+    int device = -1;
+    bool device_checked = false;
+    cplx *tw[3] = { nullptr, nullptr, nullptr };   // twiddle tables for 2nx, 2ny, 2nz (may alias)
+    std::vector<cplx> tw_host[3];
+    void *ws = nullptr;                 // workspace base
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    cplx *A = nullptr, *B = nullptr;
+    double *G = nullptr, *stage = nullptr;
+    size_t offA, offB, offG, offS, need_bytes;
+    bool greens_ready = false;
+    cudaStream_t setup_stream = nullptr;
+    cudaEvent_t setup_done = nullptr;
+    // profiling
+    int prof_slots = 0;                 // 0 = off; else per-pass events of the last prof_slots solves are kept
+    long long prof_count = 0;           // profiled solves issued since profiling was switched on
+    std::vector<cudaEvent_t> ev;        // prof_slots * (kNumPasses + 1) events
+    // generic-kernel launch parameters
+    int Wx, Wy, Wz;                     // tile widths for lines along x / y / z
+    size_t smem_x, smem_y, smem_z;
+};
+
+static const int kNumPasses = 5;
+static const int kMaxProfSlots = 1024;
+
+static bool is_pow2_in_range(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
+static int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static int tile_width_for(int L)
+{
+    // shared memory per tile = L * (W+1) * 16 B; keep it <= ~80 KB so two or more CTAs fit per SM,
+    // except for L = 2048 where W = 4 needs 160 KB.
+    if (L <= 512) return 8;
+    return 4;
+}
+
+static void compute_layout(dks_poisson_plan *p)
+{
+    const size_t nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
+    size_t off = 0;
+    p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1), 256);
+    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (nz + 1), 256);
+    p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
+    p->offS = off; off = align_up(off + 8 * nx * ny * nz, 256);
+    p->need_bytes = off;
+}
+
+static void bind_workspace(dks_poisson_plan *p)
+{
+    char *b = static_cast<char *>(p->ws);
+    p->A = reinterpret_cast<cplx *>(b + p->offA);
+    p->B = reinterpret_cast<cplx *>(b + p->offB);
+    p->G = reinterpret_cast<double *>(b + p->offG);
+    p->stage = reinterpret_cast<double *>(b + p->offS);
+}
+
+extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, double hx, double hy, double hz)
+{
+    if (!is_pow2_in_range(nx) || !is_pow2_in_range(ny) || !is_pow2_in_range(nz)) {
+        fail(DKS_ERR_INVALID_ARG, "mesh %dx%dx%d: every extent must be a power of two in [8, 1024]", nx, ny, nz);
+        return nullptr;
+    }
+    if (!(hx > 0) || !(hy > 0) || !(hz > 0) || !std::isfinite(hx) || !std::isfinite(hy) || !std::isfinite(hz)) {
+        fail(DKS_ERR_INVALID_ARG, "spacings must be finite and > 0 (got %g, %g, %g)", hx, hy, hz);
+        return nullptr;
+    }
+    dks_poisson_plan *p = new (std::nothrow) dks_poisson_plan();
+    if (!p) { fail(DKS_ERR_INVALID_ARG, "out of host memory"); return nullptr; }
+    p->d.nx = nx; p->d.ny = ny; p->d.nz = nz;
+    p->d.lx = ilog2(2 * nx); p->d.ly = ilog2(2 * ny); p->d.lz = ilog2(2 * nz);
+    p->d.gpitch = (nx + 1 + 7) / 8 * 8;
+    p->hx = hx; p->hy = hy; p->hz = hz;
+    p->g0_override = std::nan("");
+    const int Ls[3] = { 2 * nx, 2 * ny, 2 * nz };
+    for (int a = 0; a < 3; ++a) {
+        // tw[k] = exp(-2 pi i k / L), each entry straight from cosl/sinl with the argument reduced to
+        // the first octant so that the table is exactly symmetric.
+        const int L = Ls[a];
+        p->tw_host[a].resize(L);
+        const long double two_pi = 6.283185307179586476925286766559005768L;
+        for (int k = 0; k < L; ++k) {
+            long double th = two_pi * (long double)k / (long double)L;
+            p->tw_host[a][k] = make_double2((double)cosl(th), (double)(-sinl(th)));
+        }
+    }
+    // tile widths: lines along x are tiled over ky (2ny >= 16 of them per plane); lines along y / z are
+    // tiled over x (nx complex columns, or nx/2 packed real pairs for the z passes)
+    p->Wx = tile_width_for(2 * nx);
+    p->Wy = std::min(tile_width_for(2 * ny), nx);
+    p->Wz = std::min(tile_width_for(2 * nz), nx / 2);
+    p->smem_x = (size_t)2 * nx * (p->Wx + 1) * sizeof(cplx);
+    p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
+    p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
+    compute_layout(p);
+    g_err[0] = 0;
+    return p;
+}
+
+static void release_device(dks_poisson_plan *p)
+{
+    for (int a = 0; a < 3; ++a) {
+        bool alias = false;
+        for (int b = 0; b < a; ++b) alias |= (p->tw[b] == p->tw[a]);
+        if (p->tw[a] && !alias) cudaFree(p->tw[a]);
+    }
+    for (int a = 0; a < 3; ++a) p->tw[a] = nullptr;
+    if (p->ws_owned && p->ws) cudaFree(p->ws);
+    p->ws = nullptr; p->ws_owned = false;
+    if (p->setup_done) cudaEventDestroy(p->setup_done);
+    p->setup_done = nullptr;
+    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    p->ev.clear();
+}
+
+extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
+{
+    if (!p) return;
+    release_device(p);
+    delete p;
+}
+
+// First device touch: check the architecture, upload twiddles, create events, opt in to large smem.
+static int ensure_device(dks_poisson_plan *p)
+{
+    if (p->device_checked) return DKS_OK;
+    int dev = 0;
+    DKS_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    DKS_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device %d (%s) is compute capability %d.%d; this library is built for sm_100a only",
+                    dev, prop.name, prop.major, prop.minor);
+    p->device = dev;
+    const int Ls[3] = { 2 * p->d.nx, 2 * p->d.ny, 2 * p->d.nz };
+    for (int a = 0; a < 3; ++a) {
+        for (int b = 0; b < a; ++b) if (Ls[b] == Ls[a]) p->tw[a] = p->tw[b];
+        if (p->tw[a]) continue;
+        DKS_CUDA(cudaMalloc(&p->tw[a], sizeof(cplx) * Ls[a]));
+        DKS_CUDA(cudaMemcpy(p->tw[a], p->tw_host[a].data(), sizeof(cplx) * Ls[a], cudaMemcpyHostToDevice));
+    }
+    DKS_CUDA(cudaEventCreateWithFlags(&p->setup_done, cudaEventDisableTiming));
+    const size_t smem_max = std::max(p->smem_x, std::max(p->smem_y, p->smem_z));
+    const size_t smem_g = (size_t)2 * std::max(p->d.nx, std::max(p->d.ny, p->d.nz)) * (4 + 1) * sizeof(cplx);
+    if ((size_t)prop.sharedMemPerBlockOptin < std::max(smem_max, smem_g))
+        return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device offers %zu B of shared memory per block, %zu needed",
+                    (size_t)prop.sharedMemPerBlockOptin, std::max(smem_max, smem_g));
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_z));
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_z));
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_y));
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_y));
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_x));
+    DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g));
+    p->device_checked = true;
+    return DKS_OK;
+}
+
+extern "C" size_t dks_poisson_workspace_bytes(const dks_poisson_plan *p)
+{
+    if (!p) { fail(DKS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
+    return p->need_bytes;
+}
+
+extern "C" int dks_poisson_set_workspace(dks_poisson_plan *p, void *dev_ptr, size_t bytes)
+{
+    if (!p || !dev_ptr) return fail(DKS_ERR_INVALID_ARG, "plan or workspace pointer is NULL");
+    if (reinterpret_cast<uintptr_t>(dev_ptr) % 256) return fail(DKS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (bytes < p->need_bytes)
+        return fail(DKS_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, p->need_bytes);
+    if (p->ws_owned && p->ws) cudaFree(p->ws);
+    p->ws = dev_ptr; p->ws_bytes = bytes; p->ws_owned = false;
+    bind_workspace(p);
+    p->greens_ready = false;
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_stream(dks_poisson_plan *p, void *stream)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    p->setup_stream = static_cast<cudaStream_t>(stream);
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_spacing(dks_poisson_plan *p, double hx, double hy, double hz)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (!(hx > 0) || !(hy > 0) || !(hz > 0) || !std::isfinite(hx) || !std::isfinite(hy) || !std::isfinite(hz))
+        return fail(DKS_ERR_INVALID_ARG, "spacings must be finite and > 0 (got %g, %g, %g)", hx, hy, hz);
+    p->hx = hx; p->hy = hy; p->hz = hz;
+    p->greens_ready = false;
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_g0(dks_poisson_plan *p, double g0)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (std::isinf(g0)) return fail(DKS_ERR_INVALID_ARG, "g0 must be finite or NaN");
+    p->g0_override = g0;
+    p->greens_ready = false;
+    return DKS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0: Green's function build + transform
+// ------------------------------------------------------------------------------------------------
+extern "C" int dks_greens_setup(dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    if (!p->ws) {
+        DKS_CUDA(cudaMalloc(&p->ws, p->need_bytes));
+        p->ws_bytes = p->need_bytes; p->ws_owned = true;
+        bind_workspace(p);
+    }
+    const MeshDims d = p->d;
+    cudaStream_t st = p->setup_stream;
+    // 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), evaluated in long double.
+    const long double pi_l = 3.141592653589793238462643383279502884L;
+    const double coef = (double)(1.0L / (4.0L * pi_l * 8.8541878128e-12L));
+    const double hmin = std::min(p->hx, std::min(p->hy, p->hz));
+    const double g0 = std::isnan(p->g0_override) ? coef / (0.5 * hmin) : p->g0_override;
+    {
+        dim3 blk(128), grd((d.nx + 1 + 127) / 128, d.ny + 1, d.nz + 1);
+        greens_fill_kernel<<<grd, blk, 0, st>>>(p->G, d, p->hx, p->hy, p->hz, coef, g0);
+    }
+    const long long pitch = d.gpitch, plane = pitch * (d.ny + 1);
+    const int W = 4;
+    // x lines: (ky, kz) ; y lines: (kx, kz) ; z lines: (kx, ky)
+    {
+        long long nl = (long long)(d.ny + 1) * (d.nz + 1);
+        size_t sm = (size_t)2 * d.nx * (W + 1) * sizeof(cplx);
+        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.nx, d.lx, W, 1, d.ny + 1, pitch,
+                                                                         d.nz + 1, plane, 1.0, p->tw[0]);
+    }
+    {
+        long long nl = (long long)(d.nx + 1) * (d.nz + 1);
+        size_t sm = (size_t)2 * d.ny * (W + 1) * sizeof(cplx);
+        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.ny, d.ly, W, pitch, d.nx + 1, 1,
+                                                                         d.nz + 1, plane, 1.0, p->tw[1]);
+    }
+    {
+        long long nl = (long long)(d.nx + 1) * (d.ny + 1);
+        size_t sm = (size_t)2 * d.nz * (W + 1) * sizeof(cplx);
+        // fold hx hy hz / (8 nx ny nz) (Eq. (2)'s prefactor and the inverse transform's 1/N, reading A5)
+        const double scale = p->hx * p->hy * p->hz / (8.0 * d.nx * d.ny * d.nz);
+        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.nz, d.lz, W, plane, d.nx + 1, 1,
+                                                                         d.ny + 1, pitch, scale, p->tw[2]);
+    }
+    DKS_CUDA(cudaGetLastError());
+    DKS_CUDA(cudaEventRecord(p->setup_done, st));
+    p->greens_ready = true;
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_copy_greens_hat(dks_poisson_plan *p, double *host_out)
+{
+    if (!p || !host_out) return fail(DKS_ERR_INVALID_ARG, "plan or output pointer is NULL");
+    if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "dks_greens_setup has not been called");
+    DKS_CUDA(cudaEventSynchronize(p->setup_done));
+    const MeshDims d = p->d;
+    DKS_CUDA(cudaMemcpy2D(host_out, sizeof(double) * (d.nx + 1), p->G, sizeof(double) * d.gpitch,
+                          sizeof(double) * (d.nx + 1), (size_t)(d.ny + 1) * (d.nz + 1), cudaMemcpyDeviceToHost));
+    return DKS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// the solve
+// ------------------------------------------------------------------------------------------------
+extern "C" int dks_poisson_launches_per_solve(const dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    return kNumPasses;
+}
+
+extern "C" double dks_poisson_model_bytes(const dks_poisson_plan *p, int pass)
+{
+    if (!p) { fail(DKS_ERR_INVALID_ARG, "plan is NULL"); return 0.0; }
+    const double nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
+    const double rho = 8 * nx * ny * nz, a = 16 * nx * ny * (nz + 1), b = 2 * a;
+    const double g = 8 * (nx + 1) * (ny + 1) * (nz + 1);
+    switch (pass) {
+    case 0: return 2 * rho + 4 * a + 4 * b + g;
+    case 1: return rho + a;
+    case 2: return a + b;
+    case 3: return 2 * b + g;
+    case 4: return a + b;
+    case 5: return rho + a;
+    default: fail(DKS_ERR_INVALID_ARG, "pass must be 0..5"); return 0.0;
+    }
+}
+
+extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass)
+{
+    if (!p || pass < 1 || pass > 5) { fail(DKS_ERR_INVALID_ARG, "bad plan or pass"); return ""; }
+    static const char *names[5] = { "p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic",
+                                    "p4_y_inv_generic", "p5_z_c2r_generic" };
+    return names[pass - 1];
+}
+
+extern "C" int dks_poisson_set_profiling(dks_poisson_plan *p, int slots)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (slots < 0 || slots > kMaxProfSlots) return fail(DKS_ERR_INVALID_ARG, "slots must be in [0, %d]", kMaxProfSlots);
+    if (slots > 0) {
+        int rc = ensure_device(p);
+        if (rc) return rc;
+    }
+    const size_t need = (size_t)slots * (kNumPasses + 1);
+    while (p->ev.size() < need) {
+        cudaEvent_t e;
+        DKS_CUDA(cudaEventCreate(&e));
+        p->ev.push_back(e);
+    }
+    p->prof_slots = slots;
+    p->prof_count = 0;
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int count)
+{
+    if (!p || !ms_out) return fail(DKS_ERR_INVALID_ARG, "plan or output pointer is NULL");
+    if (p->prof_slots == 0 || p->prof_count == 0) return fail(DKS_ERR_NOT_SETUP, "no profiled solve has been issued");
+    const int n = std::min(count, kNumPasses);
+    const long long solves = std::min<long long>(p->prof_count, p->prof_slots);
+    std::vector<double> acc(n, 0.0);
+    for (long long s = 0; s < solves; ++s) {
+        cudaEvent_t *e = &p->ev[(size_t)s * (kNumPasses + 1)];
+        DKS_CUDA(cudaEventSynchronize(e[kNumPasses]));
+        for (int i = 0; i < n; ++i) {
+            float ms = 0.f;
+            DKS_CUDA(cudaEventElapsedTime(&ms, e[i], e[i + 1]));
+            acc[i] += ms;
+        }
+    }
+    for (int i = 0; i < n; ++i) ms_out[i] = (float)(acc[i] / (double)solves);
+    return n;
+}
+
+extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double *phi, void *stream)
+{
+    if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
+    if ((reinterpret_cast<uintptr_t>(rho) | reinterpret_cast<uintptr_t>(phi)) % 16)
+        return fail(DKS_ERR_INVALID_ARG, "rho and phi must be 16-byte aligned");
+    if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const MeshDims d = p->d;
+    if (st != p->setup_stream) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+    const bool prof = p->prof_slots > 0;
+    cudaEvent_t *ev = prof ? &p->ev[(size_t)(p->prof_count % p->prof_slots) * (kNumPasses + 1)] : nullptr;
+    if (prof) DKS_CUDA(cudaEventRecord(ev[0], st));
+    p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]);
+    if (prof) DKS_CUDA(cudaEventRecord(ev[1], st));
+    p2_y_fwd_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->A, p->B, d, p->Wy, p->tw[1]);
+    if (prof) DKS_CUDA(cudaEventRecord(ev[2], st));
+    p3_x_conv_generic<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, p->Wx,
+                                                                                                 p->tw[0]);
+    if (prof) DKS_CUDA(cudaEventRecord(ev[3], st));
+    p4_y_inv_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->B, p->A, d, p->Wy, p->tw[1]);
+    if (prof) DKS_CUDA(cudaEventRecord(ev[4], st));
+    p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]);
+    if (prof) { DKS_CUDA(cudaEventRecord(ev[5], st)); ++p->prof_count; }
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_solve_host(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
+{
+    if (!p || !rho_host || !phi_host) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
+    if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve_host");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t bytes = sizeof(double) * (size_t)p->d.nx * p->d.ny * p->d.nz;
+    DKS_CUDA(cudaMemcpyAsync(p->stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
+    int rc = dks_poisson_solve(p, p->stage, p->stage, stream);
+    if (rc) return rc;
+    DKS_CUDA(cudaMemcpyAsync(phi_host, p->stage, bytes, cudaMemcpyDeviceToHost, st));
+    DKS_CUDA(cudaStreamSynchronize(st));
+    return DKS_OK;
+}

@@ -1,0 +1,281 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances are BASELINE.json's north_star: relative L2 error <= 1e-12 and max-abs error
+<= 1e-11 * max|phi| in fp64 (definitions: SURVEY.md section 8(c) A12 / DESIGN.md).
+The oracle is the long-double build (its own error ~1e-18), so the measured error is the GPU's.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_TOL = 1e-12
+MAX_ABS_TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def dks():
+    from paper_1509_07685_b200 import dks as D
+    return D
+
+
+def gpu_solve(torch, dks, rho, n, h, g0=None):
+    plan = dks.PoissonPlan(n, h, g0=g0)
+    try:
+        d_rho = torch.from_numpy(rho).cuda()
+        d_phi = plan.solve(d_rho)
+        torch.cuda.synchronize()
+        return d_phi.cpu().numpy()
+    finally:
+        plan.close()
+
+
+def errors(got, ref):
+    rel_l2 = float(np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel()))
+    max_abs = float(np.max(np.abs(got - ref)) / np.max(np.abs(ref)))
+    return rel_l2, max_abs
+
+
+def check(got, ref):
+    assert np.all(np.isfinite(got))
+    rel_l2, max_abs = errors(got, ref)
+    assert rel_l2 <= REL_L2_TOL, f"rel-L2 {rel_l2:.3e}"
+    assert max_abs <= MAX_ABS_TOL, f"max-abs/max|phi| {max_abs:.3e}"
+    return rel_l2, max_abs
+
+
+# ---- BASELINE.json configs 1, 2, 3, 5 in full against the long-double oracle -----------------------
+@pytest.mark.parametrize("ci", [1, 2, 3, 5])
+def test_config_full_parity(torch_cuda, dks, oracle, workloads, ci):
+    w = workloads.config(ci)
+    rho = workloads.make_rho(w)
+    ref = oracle.solve(rho, w.n, w.h, precision="ld")
+    got = gpu_solve(torch_cuda, dks, rho, w.n, w.h)
+    rel_l2, max_abs = check(got, ref)
+    print(f"{w.name}: rel-L2 {rel_l2:.3e}  max-abs/max {max_abs:.3e}")
+
+
+# ---- config 4 (256^3), the bench configuration ----------------------------------------------------
+# The long-double oracle needs 2 x 4.3 GB and minutes on this size, so at full size the GPU result is
+# checked (a) at the 73 stored nodes against the direct summation of Eq. (2) (tests/golden/, written by
+# oracle/ only), (b) at ~200 more sampled nodes against direct summation computed now, (c) in full
+# against the double-precision oracle build (error ~1e-15, far below the tolerance).
+def test_config4_sampled_parity(torch_cuda, dks, oracle, workloads):
+    import os
+    w = workloads.config(4)
+    rho = workloads.make_rho(w)
+    got = gpu_solve(torch_cuda, dks, rho, w.n, w.h)
+    assert np.all(np.isfinite(got))
+    a = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "sampled_phi_cfg4.txt"))
+    nodes, direct = a[:, :3].astype(np.int64), a[:, 3]
+    g = got[nodes[:, 2], nodes[:, 1], nodes[:, 0]]
+    scale = np.max(np.abs(got))
+    assert np.max(np.abs(g - direct)) <= MAX_ABS_TOL * scale
+    assert np.max(np.abs(g - direct) / np.abs(direct)) <= 1e-11
+    more = workloads.sample_nodes(w.n, 12345, count=32)
+    d2 = oracle.direct_sum_nodes(rho, w.n, w.h, more)
+    g2 = got[more[:, 2], more[:, 1], more[:, 0]]
+    assert np.max(np.abs(g2 - d2)) <= MAX_ABS_TOL * scale
+
+
+@pytest.mark.slow
+def test_config4_full_parity_double_oracle(torch_cuda, dks, oracle, workloads):
+    w = workloads.config(4)
+    rho = workloads.make_rho(w)
+    ref = oracle.solve(rho, w.n, w.h, precision="d")
+    got = gpu_solve(torch_cuda, dks, rho, w.n, w.h)
+    rel_l2, max_abs = check(got, ref)
+    print(f"{w.name}: rel-L2 {rel_l2:.3e}  max-abs/max {max_abs:.3e}")
+
+
+# ---- shapes: every axis length class, non-cubic, anisotropic h, smallest and ragged cases ---------------
+SHAPES = [
+    ((8, 8, 8), (1e-3, 1e-3, 1e-3)),
+    ((8, 16, 32), (1e-3, 2e-3, 5e-4)),
+    ((32, 8, 16), (3e-4, 1e-3, 2e-3)),
+    ((16, 64, 8), (1e-3, 1e-3, 1e-3)),
+    ((64, 32, 128), (2e-4, 3e-4, 1e-4)),
+    ((128, 16, 64), (1e-4, 1e-4, 4e-4)),
+    ((32, 256, 16), (1e-3, 1e-4, 1e-3)),
+    ((256, 8, 8), (1e-4, 1e-3, 1e-3)),
+    ((8, 8, 512), (1e-3, 1e-3, 5e-5)),
+    ((16, 512, 8), (1e-3, 5e-5, 1e-3)),
+    ((512, 8, 16), (5e-5, 1e-3, 1e-3)),
+    ((8, 8, 1024), (1e-3, 1e-3, 2e-5)),
+    ((1024, 8, 8), (2e-5, 1e-3, 1e-3)),
+    ((8, 1024, 8), (1e-3, 2e-5, 1e-3)),
+]
+
+
+@pytest.mark.parametrize("n,h", SHAPES)
+def test_shapes_signed_random(torch_cuda, dks, oracle, workloads, n, h):
+    rho = workloads.random_rho(n, seed=sum(n))
+    ref = oracle.solve(rho, n, h, precision="ld")
+    got = gpu_solve(torch_cuda, dks, rho, n, h)
+    check(got, ref)
+
+
+# ---- degenerate inputs -------------------------------------------------------------------------------
+def test_zero_rho_gives_zero_phi(torch_cuda, dks):
+    n, h = (16, 16, 16), (1e-3, 1e-3, 1e-3)
+    got = gpu_solve(torch_cuda, dks, np.zeros((16, 16, 16)), n, h)
+    assert np.all(got == 0.0)
+
+
+@pytest.mark.parametrize("src", [(0, 0, 0), (15, 31, 7), (7, 13, 3)])
+def test_point_charge(torch_cuda, dks, oracle, src):
+    # rho = q/(hx hy hz) at one node -> phi = q G(x - s), phi[s] = q g0 (PAPER.md:121 with one term)
+    n, h = (16, 32, 8), (1e-3, 5e-4, 2e-3)
+    nx, ny, nz = n
+    q = 1e-9
+    rho = np.zeros((nz, ny, nx))
+    rho[src[2], src[1], src[0]] = q / (h[0] * h[1] * h[2])
+    got = gpu_solve(torch_cuda, dks, rho, n, h)
+    ref = oracle.solve(rho, n, h, precision="ld")
+    check(got, ref)
+    far = (nx - 1 - src[0], ny - 1 - src[1], nz - 1 - src[2])
+    if far != src:
+        g = q * oracle.green((far[0] - src[0]) * h[0], (far[1] - src[1]) * h[1], (far[2] - src[2]) * h[2])
+        assert abs(got[far[2], far[1], far[0]] - g) <= 1e-11 * np.max(np.abs(got))
+    assert abs(got[src[2], src[1], src[0]] - q * oracle.default_g0(h)) <= 1e-11 * np.max(np.abs(got))
+
+
+def test_g0_override_and_spacing_change(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    n, h1, h2 = (16, 16, 32), (1e-3, 1e-3, 1e-3), (2e-3, 1e-3, 5e-4)
+    rho = workloads.random_rho(n, seed=5, signed=False)
+    plan = dks.PoissonPlan(n, h1, g0=123.0)
+    try:
+        d_rho = torch.from_numpy(rho).cuda()
+        got1 = plan.solve(d_rho).cpu().numpy()
+        check(got1, oracle.solve(rho, n, h1, g0=123.0, precision="ld"))
+        dks.dks_poisson_set_g0(plan.handle, float("nan"))
+        # spacing changed: solve must refuse until the Green's transform is rebuilt
+        dks.dks_poisson_set_spacing(plan.handle, *h2)
+        with pytest.raises(dks.DksError) as e:
+            dks.dks_poisson_solve(plan.handle, d_rho, d_rho, None)
+        assert e.value.status == dks.DKS_ERR_NOT_SETUP
+        plan.set_spacing(h2)
+        got2 = plan.solve(d_rho).cpu().numpy()
+        check(got2, oracle.solve(rho, n, h2, precision="ld"))
+    finally:
+        plan.close()
+
+
+def test_in_place_and_repeatable(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    w = workloads.config(2)
+    rho = workloads.make_rho(w)
+    plan = dks.PoissonPlan(w.n, w.h)
+    try:
+        d = torch.from_numpy(rho).cuda()
+        out1 = plan.solve(d).clone()
+        out2 = plan.solve(d).clone()
+        assert torch.equal(out1, out2)                       # deterministic, no hidden state
+        buf = d.clone()
+        plan.solve(buf, buf)                                 # phi aliases rho
+        assert torch.equal(buf, out1)
+    finally:
+        plan.close()
+
+
+def test_greens_hat_matches_oracle_transform(torch_cuda, dks, oracle):
+    # Ghat octant (scale folded in) against numpy's FFT of the oracle-independent definition is NOT
+    # used here; instead: solve of a unit point charge at the origin returns exactly G on the mesh.
+    n, h = (16, 16, 16), (1e-3, 2e-3, 5e-4)
+    rho = np.zeros((16, 16, 16))
+    rho[0, 0, 0] = 1.0 / (h[0] * h[1] * h[2])
+    got = gpu_solve(torch_cuda, dks, rho, n, h)
+    for (i, j, k) in [(1, 0, 0), (0, 1, 0), (0, 0, 1), (3, 4, 5), (15, 15, 15)]:
+        g = oracle.green(i * h[0], j * h[1], k * h[2])
+        assert abs(got[k, j, i] - g) <= 1e-11 * np.max(np.abs(got))
+
+
+def test_solve_host_path(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    w = workloads.config(1)
+    rho = workloads.make_rho(w)
+    plan = dks.PoissonPlan(w.n, w.h)
+    try:
+        h_rho = torch.from_numpy(rho).pin_memory()
+        h_phi = torch.empty_like(h_rho).pin_memory()
+        plan.solve_host(h_rho, h_phi)
+        check(h_phi.numpy(), oracle.solve(rho, w.n, w.h, precision="ld"))
+    finally:
+        plan.close()
+
+
+def test_stream_ordering_and_graph_capture(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    w = workloads.config(1)
+    rho = workloads.make_rho(w)
+    ref = oracle.solve(rho, w.n, w.h, precision="ld")
+    plan = dks.PoissonPlan(w.n, w.h)
+    try:
+        s = torch.cuda.Stream()
+        d_rho = torch.from_numpy(rho).cuda()
+        d_phi = torch.empty_like(d_rho)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            plan.solve(d_rho, d_phi)
+        s.synchronize()
+        check(d_phi.cpu().numpy(), ref)
+        # CUDA-graph capture of the solve (stream-ordered, no allocation, no sync inside)
+        d_phi.zero_()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            plan.solve(d_rho, d_phi)
+        g.replay()
+        torch.cuda.synchronize()
+        check(d_phi.cpu().numpy(), ref)
+    finally:
+        plan.close()
+
+
+def test_caller_owned_and_plan_owned_workspace(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    n, h = (16, 16, 16), (1e-3, 1e-3, 1e-3)
+    rho = workloads.random_rho(n, seed=3)
+    ref = oracle.solve(rho, n, h, precision="ld")
+    d_rho = torch.from_numpy(rho).cuda()
+    # plan-owned workspace (allocated at setup, not in solve)
+    p = dks.PoissonPlan(n, h, own_workspace=False)
+    try:
+        check(p.solve(d_rho).cpu().numpy(), ref)
+    finally:
+        p.close()
+    # too-small caller workspace is refused
+    h_ = dks.dks_poisson_plan_create(*n, *h)
+    try:
+        small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+        with pytest.raises(dks.DksError) as e:
+            dks.dks_poisson_set_workspace(h_, small, 1024)
+        assert e.value.status == dks.DKS_ERR_WORKSPACE_TOO_SMALL
+        with pytest.raises(dks.DksError) as e:
+            dks.dks_poisson_solve(h_, d_rho, d_rho, None)
+        assert e.value.status == dks.DKS_ERR_NOT_SETUP
+    finally:
+        dks.dks_poisson_plan_destroy(h_)
+
+
+def test_pass_times_and_names(torch_cuda, dks, workloads):
+    torch = torch_cuda
+    w = workloads.config(2)
+    plan = dks.PoissonPlan(w.n, w.h)
+    try:
+        d = torch.from_numpy(workloads.make_rho(w)).cuda()
+        dks.dks_poisson_set_profiling(plan.handle, True)
+        plan.solve(d)
+        t = dks.dks_poisson_pass_times(plan.handle)
+        assert len(t) == 5 and all(x > 0 for x in t)
+        assert all(dks.dks_poisson_pass_name(plan.handle, i) for i in range(1, 6))
+        assert dks.dks_poisson_launches_per_solve(plan.handle) >= 1
+    finally:
+        plan.close()
