@@ -63,6 +63,7 @@ struct dks_poisson_plan {
     double *G = nullptr, *stage = nullptr;
     size_t offA, offB, offG, offS, need_bytes;
     bool greens_ready = false;
+    bool setup_pending = false;         // setup_done not yet known to have completed
     cudaStream_t setup_stream = nullptr;
     cudaEvent_t setup_done = nullptr;
     // profiling
@@ -304,6 +305,7 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
     DKS_CUDA(cudaGetLastError());
     DKS_CUDA(cudaEventRecord(p->setup_done, st));
     p->greens_ready = true;
+    p->setup_pending = true;
     return DKS_OK;
 }
 
@@ -399,7 +401,24 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const MeshDims d = p->d;
-    if (st != p->setup_stream) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+    if (p->setup_pending) {
+        // Order this solve after the Green's setup.  A stream under capture must not wait on work
+        // recorded outside the capture, so there the host waits for the setup instead (once).
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        DKS_CUDA(cudaStreamIsCapturing(st, &cs));
+        if (cs != cudaStreamCaptureStatusNone) {
+            cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+            DKS_CUDA(cudaThreadExchangeStreamCaptureMode(&mode));
+            cudaError_t e = cudaEventSynchronize(p->setup_done);
+            DKS_CUDA(cudaThreadExchangeStreamCaptureMode(&mode));
+            DKS_CUDA(e);
+            p->setup_pending = false;
+        } else {
+            if (st != p->setup_stream) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+            if (cudaEventQuery(p->setup_done) == cudaSuccess) p->setup_pending = false;
+            else (void)cudaGetLastError();   // cudaErrorNotReady is not a failure
+        }
+    }
     const bool prof = p->prof_slots > 0;
     cudaEvent_t *ev = prof ? &p->ev[(size_t)(p->prof_count % p->prof_slots) * (kNumPasses + 1)] : nullptr;
     if (prof) DKS_CUDA(cudaEventRecord(ev[0], st));
