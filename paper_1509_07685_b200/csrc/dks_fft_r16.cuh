@@ -1,0 +1,187 @@
+// Register-resident FFT building blocks for the specialised passes (dks_passes_r16.cuh).
+//
+// A padded line of length L = 2n (n = mesh extent = 16 A, A in {2,4,8,16}) is never transformed as a
+// whole.  PAPER.md:98 zero-pads rho to the doubled domain; a radix-2 decimation-in-frequency step on
+// a line whose upper half is zero is free:
+//     X[2K + p] = FFT_n( x[m] * w_L^(p m) )[K],   p = 0,1  (w_L = exp(-2 pi i / L)),
+// and the crop after the inverse transform makes the last decimation-in-time step half as long:
+//     y[m] = IFFT_n(X[2K])[m] + w_L^(-m) IFFT_n(X[2K+1])[m],   m < n.
+// So every padded line is two length-n sub-transforms ("parities" p = 0,1) run by 2A threads.
+//
+// One sub-transform of length n = 16 A is a four-step FFT over A threads x 16 registers:
+//   element m = a + A b lives in thread a, register b (the same mapping on input and on output);
+//   radix-16 over b in registers -> twiddle w_n^(a k_b) -> transpose through shared memory
+//   -> radix-A over a in registers (16/A independent butterflies per thread).
+// The exchange itself (addressing, barrier) belongs to the pass kernels: lanes are laid out
+// differently for contiguous and for strided lines.
+#pragma once
+#include "dks_common.cuh"
+
+namespace dks {
+
+// multiply by SIGN * i
+template <int SIGN>
+__device__ __forceinline__ cplx mul_si(cplx a) { return SIGN < 0 ? cmake(a.y, -a.x) : cmake(-a.y, a.x); }
+
+// cos, sin of 2 pi m / 16
+__device__ __forceinline__ constexpr double cos16(int m)
+{
+    return m == 0 ? 1.0 : m == 1 ? 0.92387953251128675613 : m == 2 ? 0.70710678118654752440
+         : m == 3 ? 0.38268343236508977173 : m == 4 ? 0.0 : m == 5 ? -0.38268343236508977173
+         : m == 6 ? -0.70710678118654752440 : m == 7 ? -0.92387953251128675613 : m == 8 ? -1.0
+         : -cos16(m - 8);
+}
+__device__ __forceinline__ constexpr double sin16(int m)
+{
+    return m == 0 ? 0.0 : m == 1 ? 0.38268343236508977173 : m == 2 ? 0.70710678118654752440
+         : m == 3 ? 0.92387953251128675613 : m == 4 ? 1.0 : m == 5 ? 0.92387953251128675613
+         : m == 6 ? 0.70710678118654752440 : m == 7 ? 0.38268343236508977173 : m == 8 ? 0.0
+         : -sin16(m - 8);
+}
+
+// a * exp(SIGN 2 pi i M / 16), M a compile-time constant
+template <int SIGN, int M>
+__device__ __forceinline__ cplx mul_w16(cplx a)
+{
+    constexpr int m = M & 15;
+    if (m == 0) return a;
+    if (m == 4) return mul_si<SIGN>(a);
+    if (m == 8) return cmake(-a.x, -a.y);
+    if (m == 12) return mul_si<-SIGN>(a);
+    constexpr double c = cos16(m), s = SIGN * sin16(m);
+    return cmake(fma(a.x, c, -(a.y * s)), fma(a.x, s, a.y * c));
+}
+
+template <int SIGN>
+__device__ __forceinline__ void bfly2(cplx &x0, cplx &x1)
+{
+    cplx t = x0;
+    x0 = cadd(t, x1);
+    x1 = csub(t, x1);
+}
+
+// 4-point DFT, natural order in and out: x_k <- sum_n x_n exp(SIGN 2 pi i n k / 4)
+template <int SIGN>
+__device__ __forceinline__ void bfly4(cplx &x0, cplx &x1, cplx &x2, cplx &x3)
+{
+    cplx apc = cadd(x0, x2), amc = csub(x0, x2), bpd = cadd(x1, x3), bmd = mul_si<SIGN>(csub(x1, x3));
+    x0 = cadd(apc, bpd);
+    x1 = cadd(amc, bmd);
+    x2 = csub(apc, bpd);
+    x3 = csub(amc, bmd);
+}
+
+// 8-point DFT on v[0], v[S], ..., v[7S], natural order in and out
+template <int SIGN, int S>
+__device__ __forceinline__ void bfly8(cplx *v)
+{
+    bfly4<SIGN>(v[0], v[2 * S], v[4 * S], v[6 * S]);      // y0[k0] in slots 0,2,4,6
+    bfly4<SIGN>(v[1 * S], v[3 * S], v[5 * S], v[7 * S]);  // y1[k0] in slots 1,3,5,7
+    v[3 * S] = mul_w16<SIGN, 2>(v[3 * S]);
+    v[5 * S] = mul_w16<SIGN, 4>(v[5 * S]);
+    v[7 * S] = mul_w16<SIGN, 6>(v[7 * S]);
+    cplx o[8];
+#pragma unroll
+    for (int k0 = 0; k0 < 4; ++k0) {
+        o[k0] = cadd(v[2 * k0 * S], v[(2 * k0 + 1) * S]);
+        o[k0 + 4] = csub(v[2 * k0 * S], v[(2 * k0 + 1) * S]);
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k * S] = o[k];
+}
+
+// 16-point DFT in registers, natural order in and out (4 x 4 decomposition, 160 fp64 instructions)
+template <int SIGN>
+__device__ __forceinline__ void fft16(cplx (&v)[16])
+{
+#pragma unroll
+    for (int n0 = 0; n0 < 4; ++n0) bfly4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);   // slot n0 + 4 k0
+    v[5] = mul_w16<SIGN, 1>(v[5]);
+    v[9] = mul_w16<SIGN, 2>(v[9]);
+    v[13] = mul_w16<SIGN, 3>(v[13]);
+    v[6] = mul_w16<SIGN, 2>(v[6]);
+    v[10] = mul_w16<SIGN, 4>(v[10]);
+    v[14] = mul_w16<SIGN, 6>(v[14]);
+    v[7] = mul_w16<SIGN, 3>(v[7]);
+    v[11] = mul_w16<SIGN, 6>(v[11]);
+    v[15] = mul_w16<SIGN, 9>(v[15]);
+#pragma unroll
+    for (int k0 = 0; k0 < 4; ++k0) bfly4<SIGN>(v[4 * k0], v[4 * k0 + 1], v[4 * k0 + 2], v[4 * k0 + 3]);
+    // slot 4 k0 + k1 holds X[k0 + 4 k1]: transpose the 4 x 4 register tile
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = i + 1; j < 4; ++j) {
+            cplx t = v[4 * i + j];
+            v[4 * i + j] = v[4 * j + i];
+            v[4 * j + i] = t;
+        }
+}
+
+// Second step of the four-step transform: v[g A + a'] (g < 16/A) -> radix-A over a' for every g;
+// the result for k_a goes to register r = g + (16/A) k_a, i.e. sub-index tau + A r.
+template <int A, int SIGN>
+__device__ __forceinline__ void fft_second(cplx (&v)[16])
+{
+    if (A == 16) {
+        fft16<SIGN>(v);
+        return;
+    }
+    constexpr int G = 16 / A;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        if (A == 8) bfly8<SIGN, 1>(&v[g * 8]);
+        if (A == 4) bfly4<SIGN>(v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+        if (A == 2) bfly2<SIGN>(v[g * 2], v[g * 2 + 1]);
+    }
+    cplx o[16];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ka = 0; ka < A; ++ka) o[g + G * ka] = v[g * A + ka];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = o[r];
+}
+
+// twiddle between the two steps: v[k] *= w_n^(a k), table tw1[k A + a] = exp(-2 pi i a k / n)
+template <int A, int SIGN>
+__device__ __forceinline__ void twiddle_between(cplx (&v)[16], const cplx *__restrict__ tw1, int a)
+{
+#pragma unroll
+    for (int k = 1; k < 16; ++k) {
+        cplx t = __ldg(&tw1[k * A + a]);
+        v[k] = SIGN < 0 ? cmul(v[k], t) : cmulc(v[k], t);
+    }
+}
+
+// parity twiddle: v[b] *= w_L^(SIGN' (a + A b)); tw2[m] = exp(-2 pi i m / L), m < n
+template <int A, int SIGN>
+__device__ __forceinline__ void twiddle_parity(cplx (&v)[16], const cplx *__restrict__ tw2, int a)
+{
+#pragma unroll
+    for (int b = 0; b < 16; ++b) {
+        cplx t = __ldg(&tw2[a + A * b]);
+        v[b] = SIGN < 0 ? cmul(v[b], t) : cmulc(v[b], t);
+    }
+}
+
+__device__ __forceinline__ cplx shfl_xor_c(cplx v, int mask)
+{
+    return cmake(__shfl_xor_sync(0xffffffffu, v.x, mask), __shfl_xor_sync(0xffffffffu, v.y, mask));
+}
+
+// Combine of the two parities after the inverse sub-transforms (crop fused): the parity-1 thread
+// holds w_L^(-m) O[m] already.  Parity 0 keeps registers r < 8, parity 1 keeps r >= 8; each sends the
+// other half to its partner lane (lane ^ MASK).  out[i] belongs to register r = i + 8 p.
+template <int MASK>
+__device__ __forceinline__ void combine_parities(const cplx (&v)[16], int p, cplx (&out)[8])
+{
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        cplx send = p ? v[i] : v[i + 8];
+        cplx mine = p ? v[i + 8] : v[i];
+        out[i] = cadd(mine, shfl_xor_c(send, MASK));
+    }
+}
+
+}  // namespace dks

@@ -17,6 +17,7 @@
 
 #include "../../include/dks_poisson.h"
 #include "dks_passes_generic.cuh"
+#include "dks_passes_r16.cuh"
 
 using namespace dks;
 
@@ -56,6 +57,12 @@ struct dks_poisson_plan {
     bool device_checked = false;
     cplx *tw[3] = { nullptr, nullptr, nullptr };   // twiddle tables for 2nx, 2ny, 2nz (may alias)
     std::vector<cplx> tw_host[3];
+    // specialised (register-resident) passes: A = n / 16 per axis (0 = axis not supported), and the
+    // between-step twiddle tables tw1[k A + a] = exp(-2 pi i a k / n), k < 16, a < A
+    int r16A[3] = { 0, 0, 0 };
+    cplx *tw1[3] = { nullptr, nullptr, nullptr };
+    std::vector<cplx> tw1_host[3];
+    bool fast[5] = { false, false, false, false, false };   // pass P1..P5 uses the r16 kernel
     void *ws = nullptr;                 // workspace base
     size_t ws_bytes = 0;
     bool ws_owned = false;
@@ -139,6 +146,24 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
             p->tw_host[a][k] = make_double2((double)cosl(th), (double)(-sinl(th)));
         }
     }
+    const int ns[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a) {
+        const int n = ns[a];
+        if (n < 32 || n > 256) continue;
+        const int A = n / 16;
+        p->r16A[a] = A;
+        p->tw1_host[a].resize(n);
+        const long double two_pi = 6.283185307179586476925286766559005768L;
+        for (int k = 0; k < 16; ++k)
+            for (int t = 0; t < A; ++t) {
+                long double th = two_pi * (long double)((t * k) % n) / (long double)n;
+                p->tw1_host[a][k * A + t] = make_double2((double)cosl(th), (double)(-sinl(th)));
+            }
+    }
+    // P1/P5 run along z and need 16 real columns per CTA; P2/P4 along y; P3 along x (nx = 256 only)
+    p->fast[0] = p->fast[4] = p->r16A[2] != 0 && nx >= 16;
+    p->fast[1] = p->fast[3] = p->r16A[1] != 0;
+    p->fast[2] = p->r16A[0] == 16;
     // tile widths: lines along x are tiled over ky (2ny >= 16 of them per plane); lines along y / z are
     // tiled over x (nx complex columns, or nx/2 packed real pairs for the z passes)
     p->Wx = tile_width_for(2 * nx);
@@ -160,6 +185,10 @@ static void release_device(dks_poisson_plan *p)
         if (p->tw[a] && !alias) cudaFree(p->tw[a]);
     }
     for (int a = 0; a < 3; ++a) p->tw[a] = nullptr;
+    for (int a = 0; a < 3; ++a) {
+        if (p->tw1[a]) cudaFree(p->tw1[a]);     // never aliased
+        p->tw1[a] = nullptr;
+    }
     if (p->ws_owned && p->ws) cudaFree(p->ws);
     p->ws = nullptr; p->ws_owned = false;
     if (p->setup_done) cudaEventDestroy(p->setup_done);
@@ -173,6 +202,53 @@ extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
     if (!p) return;
     release_device(p);
     delete p;
+}
+
+// ------------------------------------------------------------------------------------------------
+// specialised passes: attribute setup and launch by A = n / 16
+// ------------------------------------------------------------------------------------------------
+#define DKS_FOR_EACH_A(X) X(2) X(4) X(8) X(16)
+
+static int r16_set_attributes()
+{
+#define X(A_)                                                                                                         \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
+    DKS_FOR_EACH_A(X)
+#undef X
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Warps * kP3SmemPerWarp));
+    return DKS_OK;
+}
+
+template <int A>
+static void launch_strided_r16(int pass, const dks_poisson_plan *p, const double *rho, double *phi, cudaStream_t st)
+{
+    const MeshDims d = p->d;
+    const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
+    switch (pass) {
+    case 1: p1_z_r2c_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(rho, p->A, d, p->tw1[2], p->tw[2]); break;
+    case 2: p2_y_fwd_r16<A><<<dim3(d.nx / kCols, d.nz + 1), T, S, st>>>(p->A, p->B, d, p->tw1[1], p->tw[1]); break;
+    case 4: p4_y_inv_r16<A><<<dim3(d.nx / kCols, d.nz + 1), T, S, st>>>(p->B, p->A, d, p->tw1[1], p->tw[1]); break;
+    case 5: p5_z_c2r_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(p->A, phi, d, p->tw1[2], p->tw[2]); break;
+    }
+}
+
+static void launch_r16(int pass, const dks_poisson_plan *p, const double *rho, double *phi, cudaStream_t st)
+{
+    if (pass == 3) {
+        const MeshDims d = p->d;
+        p3_x_conv_r16<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / kP3Warps), kP3Warps * 32, kP3Warps * kP3SmemPerWarp, st>>>(
+            p->B, p->G, d, p->tw1[0], p->tw[0]);
+        return;
+    }
+    const int A = (pass == 1 || pass == 5) ? p->r16A[2] : p->r16A[1];
+    switch (A) {
+#define X(A_) case A_: launch_strided_r16<A_>(pass, p, rho, phi, st); break;
+        DKS_FOR_EACH_A(X)
+#undef X
+    }
 }
 
 // First device touch: check the architecture, upload twiddles, create events, opt in to large smem.
@@ -194,6 +270,12 @@ static int ensure_device(dks_poisson_plan *p)
         DKS_CUDA(cudaMalloc(&p->tw[a], sizeof(cplx) * Ls[a]));
         DKS_CUDA(cudaMemcpy(p->tw[a], p->tw_host[a].data(), sizeof(cplx) * Ls[a], cudaMemcpyHostToDevice));
     }
+    for (int a = 0; a < 3; ++a) {
+        if (!p->r16A[a] || p->tw1[a]) continue;
+        const size_t bytes = sizeof(cplx) * p->tw1_host[a].size();
+        DKS_CUDA(cudaMalloc(&p->tw1[a], bytes));
+        DKS_CUDA(cudaMemcpy(p->tw1[a], p->tw1_host[a].data(), bytes, cudaMemcpyHostToDevice));
+    }
     DKS_CUDA(cudaEventCreateWithFlags(&p->setup_done, cudaEventDisableTiming));
     const size_t smem_max = std::max(p->smem_x, std::max(p->smem_y, p->smem_z));
     const size_t smem_g = (size_t)2 * std::max(p->d.nx, std::max(p->d.ny, p->d.nz)) * (4 + 1) * sizeof(cplx);
@@ -206,6 +288,8 @@ static int ensure_device(dks_poisson_plan *p)
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_y));
     DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_x));
     DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g));
+    int rc = r16_set_attributes();
+    if (rc) return rc;
     p->device_checked = true;
     return DKS_OK;
 }
@@ -351,7 +435,8 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     if (!p || pass < 1 || pass > 5) { fail(DKS_ERR_INVALID_ARG, "bad plan or pass"); return ""; }
     static const char *names[5] = { "p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic",
                                     "p4_y_inv_generic", "p5_z_c2r_generic" };
-    return names[pass - 1];
+    static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
+    return p->fast[pass - 1] ? fast_names[pass - 1] : names[pass - 1];
 }
 
 extern "C" int dks_poisson_set_profiling(dks_poisson_plan *p, int slots)
@@ -422,16 +507,21 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
     const bool prof = p->prof_slots > 0;
     cudaEvent_t *ev = prof ? &p->ev[(size_t)(p->prof_count % p->prof_slots) * (kNumPasses + 1)] : nullptr;
     if (prof) DKS_CUDA(cudaEventRecord(ev[0], st));
-    p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]);
+    if (p->fast[0]) launch_r16(1, p, rho, phi, st);
+    else p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]);
     if (prof) DKS_CUDA(cudaEventRecord(ev[1], st));
-    p2_y_fwd_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->A, p->B, d, p->Wy, p->tw[1]);
+    if (p->fast[1]) launch_r16(2, p, rho, phi, st);
+    else p2_y_fwd_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->A, p->B, d, p->Wy, p->tw[1]);
     if (prof) DKS_CUDA(cudaEventRecord(ev[2], st));
-    p3_x_conv_generic<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, p->Wx,
-                                                                                                 p->tw[0]);
+    if (p->fast[2]) launch_r16(3, p, rho, phi, st);
+    else p3_x_conv_generic<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, p->Wx,
+                                                                                                      p->tw[0]);
     if (prof) DKS_CUDA(cudaEventRecord(ev[3], st));
-    p4_y_inv_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->B, p->A, d, p->Wy, p->tw[1]);
+    if (p->fast[3]) launch_r16(4, p, rho, phi, st);
+    else p4_y_inv_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->B, p->A, d, p->Wy, p->tw[1]);
     if (prof) DKS_CUDA(cudaEventRecord(ev[4], st));
-    p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]);
+    if (p->fast[4]) launch_r16(5, p, rho, phi, st);
+    else p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]);
     if (prof) { DKS_CUDA(cudaEventRecord(ev[5], st)); ++p->prof_count; }
     DKS_CUDA(cudaGetLastError());
     return DKS_OK;
