@@ -162,12 +162,25 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
     const int nx = d.nx, ny = d.ny, y = blockIdx.y;
     const size_t x0 = (size_t)blockIdx.x * 2 * kCols;
-    for (int idx = tid; idx < (N + 1) * kCols; idx += THREADS) {
-        const int k = idx >> 3, cc = idx & 7;
-        const cplx *in = &Ain[((size_t)k * ny + y) * nx + x0 + 2 * cc];
-        const cplx fa = ldg_stream(in), fb = ldg_stream(in + 1);
-        ex[k * kCols + cc] = cmake(fa.x - fb.y, fa.y + fb.x);
-        if (k > 0 && k < N) ex[(L - k) * kCols + cc] = cmake(fa.x + fb.y, fb.x - fa.y);
+    // all loads of the tile in flight at once (the last round is ragged: row k = N only)
+    constexpr int ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
+    cplx fa[ROUNDS], fb[ROUNDS];
+#pragma unroll
+    for (int i = 0; i < ROUNDS; ++i) {
+        const int idx = tid + i * THREADS, k = idx >> 3, cc = idx & 7;
+        if (idx < ITEMS) {
+            const cplx *in = &Ain[((size_t)k * ny + y) * nx + x0 + 2 * cc];
+            fa[i] = ldg_stream(in);
+            fb[i] = ldg_stream(in + 1);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < ROUNDS; ++i) {
+        const int idx = tid + i * THREADS, k = idx >> 3, cc = idx & 7;
+        if (idx < ITEMS) {
+            ex[k * kCols + cc] = cmake(fa[i].x - fb[i].y, fa[i].y + fb[i].x);
+            if (k > 0 && k < N) ex[(L - k) * kCols + cc] = cmake(fa[i].x + fb[i].y, fb[i].x - fa[i].y);
+        }
     }
     __syncthreads();
     cplx v[16];
@@ -188,7 +201,8 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 // ---------------------------------------------------------------------------------------------
 constexpr int kP3Warps = 8;
 constexpr int kP3RowPad = 17;
-constexpr int kP3SmemPerWarp = 2 * 16 * kP3RowPad * (int)sizeof(cplx);
+constexpr int kP3GhatDoubles = 264;               // gpitch for nx = 256: one Ghat row, staged per warp
+constexpr int kP3SmemPerWarp = 2 * 16 * kP3RowPad * (int)sizeof(cplx) + kP3GhatDoubles * (int)sizeof(double);
 
 __global__ void __launch_bounds__(kP3Warps * 32, 2)
 p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
@@ -197,13 +211,19 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     extern __shared__ cplx smem[];
     constexpr int A = 16, N = 256, L = 512;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, a = lane & 15, p = lane >> 4;
-    cplx *ex = smem + warp * (2 * 16 * kP3RowPad) + p * 16 * kP3RowPad;
+    char *wbase = reinterpret_cast<char *>(smem) + warp * kP3SmemPerWarp;
+    cplx *ex = reinterpret_cast<cplx *>(wbase) + p * 16 * kP3RowPad;
+    double *gs = reinterpret_cast<double *>(wbase + 2 * 16 * kP3RowPad * sizeof(cplx));
     const int ny = d.ny;
-    const size_t line = (size_t)blockIdx.x * kP3Warps + warp;
-    const int kz = (int)(line / (2 * ny)), ky = (int)(line % (2 * ny));
+    const unsigned line = blockIdx.x * kP3Warps + warp;
+    const int kz = (int)(line / (unsigned)(2 * ny)), ky = (int)(line % (unsigned)(2 * ny));
     const int kyp = min(ky, 2 * ny - ky);
     const double *__restrict__ grow = Ghat + ((size_t)kz * (ny + 1) + kyp) * d.gpitch;
-    cplx *base = B + line * N;
+    // the Ghat row (nx + 1 reals, pitch 264) goes to shared memory asynchronously: it is needed only
+    // after the forward transform, and waiting for it there would expose a second DRAM latency
+    for (int i = lane; i < kP3GhatDoubles / 2; i += 32) cp_async16(gs + 2 * i, grow + 2 * i);
+    cp_async_commit();
+    cplx *base = B + (size_t)line * N;
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&base[a + A * b]);
@@ -218,11 +238,12 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * kP3RowPad + ap];
     fft16<-1>(v);
     // multiply: v[r] = X[K], K = 2 (a + 16 r) + p
+    cp_async_wait_all();
+    __syncwarp();
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int K = 2 * (a + A * r) + p;
-        const double g = __ldg(&grow[min(K, L - K)]);
-        v[r] = cscale(v[r], g);
+        v[r] = cscale(v[r], gs[min(K, L - K)]);
     }
     // inverse
     fft16<+1>(v);
