@@ -197,69 +197,118 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 
 // ---------------------------------------------------------------------------------------------
 // P3 for nx = 256: forward x, multiply by the Green's transform, inverse x, crop; in place on B.
-// One warp = one line; block = 8 warps; grid ((nz+1) * 2ny / 8).  Ghat as in the generic pass.
+// Persistent: one CTA of 12 warps per SM; every warp runs its own software pipeline over lines
+// line = warp_global + i * warps_total.  While a warp transforms line i, the bulk-copy engine brings
+// line i+1 (4 KB) and its Ghat row into the warp's shared-memory stage (cp.async.bulk + mbarrier), so
+// no DRAM latency is exposed and no register is spent on prefetching.  lane -> a = lane & 15,
+// p = lane >> 4.  The between-step twiddles depend only on the lane and stay in registers.
+// Exchange buffer per warp: ex[p][k][a ^ (k & 7)] (XOR swizzle: conflict free both ways, no padding).
 // ---------------------------------------------------------------------------------------------
-constexpr int kP3Warps = 8;
-constexpr int kP3RowPad = 17;
-constexpr int kP3GhatDoubles = 264;               // gpitch for nx = 256: one Ghat row, staged per warp
-constexpr int kP3SmemPerWarp = 2 * 16 * kP3RowPad * (int)sizeof(cplx) + kP3GhatDoubles * (int)sizeof(double);
+constexpr int kP3Warps = 12;
+constexpr int kP3GhatBytes = 2064;                 // 258 doubles >= nx + 1, multiple of 16
+constexpr int kP3OffEx = 4096;                     // after the 256-element line stage
+constexpr int kP3OffG = kP3OffEx + 8192;
+constexpr int kP3OffBar = kP3OffG + kP3GhatBytes;
+constexpr int kP3SmemPerWarp = kP3OffBar + 16;     // 14368
+constexpr int kP3SmemTw2 = 256 * (int)sizeof(cplx);
+constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp + kP3SmemTw2;
 
-__global__ void __launch_bounds__(kP3Warps * 32, 2)
+__global__ void __launch_bounds__(kP3Warps * 32, 1)
 p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
               const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
-    extern __shared__ cplx smem[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int A = 16, N = 256, L = 512;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, a = lane & 15, p = lane >> 4;
-    char *wbase = reinterpret_cast<char *>(smem) + warp * kP3SmemPerWarp;
-    cplx *ex = reinterpret_cast<cplx *>(wbase) + p * 16 * kP3RowPad;
-    double *gs = reinterpret_cast<double *>(wbase + 2 * 16 * kP3RowPad * sizeof(cplx));
-    const int ny = d.ny;
-    const unsigned line = blockIdx.x * kP3Warps + warp;
-    const int kz = (int)(line / (unsigned)(2 * ny)), ky = (int)(line % (unsigned)(2 * ny));
-    const int kyp = min(ky, 2 * ny - ky);
-    const double *__restrict__ grow = Ghat + ((size_t)kz * (ny + 1) + kyp) * d.gpitch;
-    // the Ghat row (nx + 1 reals, pitch 264) goes to shared memory asynchronously: it is needed only
-    // after the forward transform, and waiting for it there would expose a second DRAM latency
-    for (int i = lane; i < kP3GhatDoubles / 2; i += 32) cp_async16(gs + 2 * i, grow + 2 * i);
-    cp_async_commit();
-    cplx *base = B + (size_t)line * N;
-    cplx v[16];
-#pragma unroll
-    for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&base[a + A * b]);
-    // forward
-    if (p) twiddle_parity<A, -1>(v, tw2, a);
-    fft16<-1>(v);
-    twiddle_between<A, -1>(v, tw1, a);
-#pragma unroll
-    for (int k = 0; k < 16; ++k) ex[k * kP3RowPad + a] = v[k];
-    __syncwarp();
-#pragma unroll
-    for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * kP3RowPad + ap];
-    fft16<-1>(v);
-    // multiply: v[r] = X[K], K = 2 (a + 16 r) + p
-    cp_async_wait_all();
-    __syncwarp();
-#pragma unroll
-    for (int r = 0; r < 16; ++r) {
-        const int K = 2 * (a + A * r) + p;
-        v[r] = cscale(v[r], gs[min(K, L - K)]);
+    unsigned char *wb = smem_raw + warp * kP3SmemPerWarp;
+    const cplx *stage = reinterpret_cast<const cplx *>(wb);
+    cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + p * 256;
+    const double *gs = reinterpret_cast<const double *>(wb + kP3OffG);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] line data, [1] Ghat row
+    cplx *tw2s = reinterpret_cast<cplx *>(smem_raw + kP3Warps * kP3SmemPerWarp);
+    for (int i = threadIdx.x; i < 256; i += kP3Warps * 32) tw2s[i] = __ldg(&tw2[i]);
+    if (lane == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init_fence();
     }
-    // inverse
-    fft16<+1>(v);
-    twiddle_between<A, +1>(v, tw1, a);
-    __syncwarp();                                     // forward exchange reads done in every lane
+    __syncthreads();
+
+    const unsigned ny2 = 2 * d.ny, nlines = (unsigned)(d.nz + 1) * ny2, stride = gridDim.x * kP3Warps;
+    unsigned line = blockIdx.x * kP3Warps + warp;
+    auto ghat_row = [&](unsigned l) {
+        const int kz = (int)(l / ny2), ky = (int)(l % ny2);
+        return Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch;
+    };
+    if (lane == 0 && line < nlines) {
+        mbar_expect_tx(&bar[0], N * sizeof(cplx));
+        bulk_g2s(wb, B + (size_t)line * N, N * sizeof(cplx), &bar[0]);
+        mbar_expect_tx(&bar[1], kP3GhatBytes);
+        bulk_g2s(wb + kP3OffG, ghat_row(line), kP3GhatBytes, &bar[1]);
+    }
+    // between-step twiddles w_256^(a k), k = 1..15, fixed per lane
+    cplx tb[15];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) ex[k * kP3RowPad + a] = v[k];
-    __syncwarp();
+    for (int k = 1; k < 16; ++k) tb[k - 1] = __ldg(&tw1[k * A + a]);
+
+    unsigned phase = 0;
+    for (; line < nlines; line += stride, phase ^= 1) {
+        const unsigned next = line + stride;
+        cplx *base = B + (size_t)line * N;
+        cplx v[16];
+        mbar_wait(&bar[0], phase);
 #pragma unroll
-    for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * kP3RowPad + ap];
-    fft16<+1>(v);
-    if (p) twiddle_parity<A, +1>(v, tw2, a);
-    cplx out[8];
-    combine_parities<16>(v, p, out);
+        for (int b = 0; b < 16; ++b) v[b] = stage[a + A * b];
+        __syncwarp();                                 // stage consumed (and last exchange reads done)
+        if (lane == 0 && next < nlines) {
+            mbar_expect_tx(&bar[0], N * sizeof(cplx));
+            bulk_g2s(wb, B + (size_t)next * N, N * sizeof(cplx), &bar[0]);
+        }
+        // forward
+        if (p) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) stg_stream(&base[a + A * (i + 8 * p)], out[i]);
+            for (int b = 0; b < 16; ++b) v[b] = cmul(v[b], tw2s[a + A * b]);
+        }
+        fft16<-1>(v);
+#pragma unroll
+        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tb[k - 1]);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
+        __syncwarp();
+#pragma unroll
+        for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * 16 + (ap ^ (a & 7))];
+        fft16<-1>(v);
+        // multiply: v[r] = X[K], K = 2 (a + 16 r) + p
+        mbar_wait(&bar[1], phase);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int K = 2 * (a + A * r) + p;
+            v[r] = cscale(v[r], gs[min(K, L - K)]);
+        }
+        __syncwarp();                                 // Ghat row consumed, forward exchange reads done
+        if (lane == 0 && next < nlines) {
+            mbar_expect_tx(&bar[1], kP3GhatBytes);
+            bulk_g2s(wb + kP3OffG, ghat_row(next), kP3GhatBytes, &bar[1]);
+        }
+        // inverse
+        fft16<+1>(v);
+#pragma unroll
+        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tb[k - 1]);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
+        __syncwarp();
+#pragma unroll
+        for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * 16 + (ap ^ (a & 7))];
+        fft16<+1>(v);
+        if (p) {
+#pragma unroll
+            for (int b = 0; b < 16; ++b) v[b] = cmulc(v[b], tw2s[a + A * b]);
+        }
+        cplx out[8];
+        combine_parities<16>(v, p, out);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) stg_stream(&base[a + A * (i + 8 * p)], out[i]);
+    }
 }
 
 }  // namespace dks

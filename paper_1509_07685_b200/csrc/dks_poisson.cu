@@ -54,6 +54,7 @@ struct dks_poisson_plan {
     double g0_override;                 // NaN = default rule
     // device
     int device = -1;
+    int sm_count = 148;
     bool device_checked = false;
     cplx *tw[3] = { nullptr, nullptr, nullptr };   // twiddle tables for 2nx, 2ny, 2nz (may alias)
     std::vector<cplx> tw_host[3];
@@ -218,7 +219,7 @@ static int r16_set_attributes()
     DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
     DKS_FOR_EACH_A(X)
 #undef X
-    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Warps * kP3SmemPerWarp));
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem));
     return DKS_OK;
 }
 
@@ -239,8 +240,9 @@ static void launch_r16(int pass, const dks_poisson_plan *p, const double *rho, d
 {
     if (pass == 3) {
         const MeshDims d = p->d;
-        p3_x_conv_r16<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / kP3Warps), kP3Warps * 32, kP3Warps * kP3SmemPerWarp, st>>>(
-            p->B, p->G, d, p->tw1[0], p->tw[0]);
+        const unsigned lines = (unsigned)(d.nz + 1) * 2 * d.ny;
+        const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (lines + kP3Warps - 1) / kP3Warps);
+        p3_x_conv_r16<<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, p->tw1[0], p->tw[0]);
         return;
     }
     const int A = (pass == 1 || pass == 5) ? p->r16A[2] : p->r16A[1];
@@ -263,6 +265,7 @@ static int ensure_device(dks_poisson_plan *p)
         return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device %d (%s) is compute capability %d.%d; this library is built for sm_100a only",
                     dev, prop.name, prop.major, prop.minor);
     p->device = dev;
+    p->sm_count = prop.multiProcessorCount;
     const int Ls[3] = { 2 * p->d.nx, 2 * p->d.ny, 2 * p->d.nz };
     for (int a = 0; a < 3; ++a) {
         for (int b = 0; b < a; ++b) if (Ls[b] == Ls[a]) p->tw[a] = p->tw[b];
