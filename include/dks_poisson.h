@@ -67,7 +67,8 @@ int dks_greens_setup(dks_poisson_plan *plan);
 /* The hot path: phi = hx hy hz FT^-1{FT{rho} (x) FT{G}} cropped to the mesh.
  * rho_dev, phi_dev: device pointers as described above; rho_dev is only read; phi_dev may alias
  * rho_dev.  stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous and stream-ordered:
- * no host synchronisation, no allocation; CUDA-graph capturable.  Five kernel launches. */
+ * no host synchronisation, no allocation; CUDA-graph capturable.  Launches P1, then P2-P3-P4 once per
+ * slab of kz planes (dks_poisson_set_slab_planes), then P5: 2 + 3 * ceil((nz+1)/slab) kernels. */
 int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, void *stream);
 
 /* Same solve with HOST buffers (the end-to-end path of the paper: rho is copied to
@@ -83,8 +84,8 @@ int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double
 /* Overrides G(0,0,0); NaN restores the default rule.  Invalidates the Green's transform. */
 int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
 
-/* Bytes of device workspace the plan needs (buffers A, B, the Green's octant, the host-path staging
- * buffer). */
+/* Bytes of device workspace the plan needs (buffer A, the Green's octant, the host-path staging
+ * buffer, one slab of B). */
 size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
 
 /* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace; 256-byte aligned,
@@ -92,13 +93,25 @@ size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
  * Invalidates the Green's transform. */
 int dks_poisson_set_workspace(dks_poisson_plan *plan, void *dev_ptr, size_t bytes);
 
+/* P2, P3 and P4 work on independent kz planes of the half-spectrum (kz = 0..nz).  They are launched
+ * slab by slab -- `planes` consecutive kz planes at a time -- so that the buffer B between them
+ * ([planes][2ny][nx] complex) is a scratch that stays in the L2 cache instead of going through HBM.
+ * planes = 0 restores the automatic choice (about 40 MB of B per slab); planes = nz+1 is the unslabbed
+ * pipeline.  Changes dks_poisson_workspace_bytes(); call it before attaching a workspace / before
+ * dks_greens_setup (afterwards it fails with DKS_ERR_WORKSPACE_TOO_SMALL if the workspace cannot
+ * hold the new slab).  Switches per-pass profiling off.  dks_poisson_slab_planes returns the
+ * current value. */
+int dks_poisson_set_slab_planes(dks_poisson_plan *plan, int planes);
+int dks_poisson_slab_planes(const dks_poisson_plan *plan);
+
 /* Stream used by dks_greens_setup (default NULL = legacy default stream). */
 int dks_poisson_set_stream(dks_poisson_plan *plan, void *stream);
 
 /* Per-pass timing.  slots > 0: dks_poisson_solve records CUDA events on its stream around each of
- * its five passes (still asynchronous) and keeps those of the last `slots` solves (slots <= 1024);
+ * its launches (still asynchronous) and keeps those of the last `slots` solves (slots <= 256);
  * slots = 0 switches it off.  dks_poisson_pass_times waits for the recorded solves and writes up to
- * `count` durations in milliseconds (pass order P1..P5), each the mean over the recorded solves;
+ * `count` durations in milliseconds (pass order P1..P5, summed over the slabs), each the mean over the
+ * recorded solves;
  * returns the number of passes written or a negative status. */
 int dks_poisson_set_profiling(dks_poisson_plan *plan, int slots);
 int dks_poisson_pass_times(dks_poisson_plan *plan, float *ms_out, int count);

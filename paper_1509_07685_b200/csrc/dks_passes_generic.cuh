@@ -86,7 +86,7 @@ p5_z_c2r_generic(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims 
 // P2: forward y.  grid (nx / W, nz + 1)
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-p2_y_fwd_generic(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, int W,
+p2_y_fwd_generic(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, int kz0, int W,
                  const cplx *__restrict__ tw)
 {
     extern __shared__ cplx s[];
@@ -95,7 +95,7 @@ p2_y_fwd_generic(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, i
     const int tid = threadIdx.x, nt = blockDim.x;
     for (int idx = tid; idx < ny * W; idx += nt) {
         int r = idx / W, w = idx % W;
-        s[r * W + w] = A[((size_t)kz * ny + r) * nx + x0 + w];
+        s[r * W + w] = A[((size_t)(kz0 + kz) * ny + r) * nx + x0 + w];
         s[(r + ny) * W + w] = cmake(0.0, 0.0);
     }
     __syncthreads();
@@ -110,7 +110,7 @@ p2_y_fwd_generic(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, i
 // P4: inverse y, crop to ny.  grid (nx / W, nz + 1)
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-p4_y_inv_generic(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, int W,
+p4_y_inv_generic(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, int kz0, int W,
                  const cplx *__restrict__ tw)
 {
     extern __shared__ cplx s[];
@@ -125,7 +125,7 @@ p4_y_inv_generic(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, i
     tile_fft_dit<+1>(s, L, logL, W, W, tw);
     for (int idx = tid; idx < ny * W; idx += nt) {
         int r = idx / W, w = idx % W;
-        A[((size_t)kz * ny + r) * nx + x0 + w] = s[r * W + w];
+        A[((size_t)(kz0 + kz) * ny + r) * nx + x0 + w] = s[r * W + w];
     }
 }
 
@@ -136,13 +136,13 @@ p4_y_inv_generic(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, i
 // spectrum follows from evenness: Ghat(kx, ky, kz) = Ghat(min(kx, 2nx-kx), min(ky, 2ny-ky), kz).
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-p3_x_conv_generic(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int W,
+p3_x_conv_generic(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, int W,
                   const cplx *__restrict__ tw)
 {
     extern __shared__ cplx s[];
     const int nx = d.nx, ny = d.ny, L = 2 * nx, logL = d.lx, WP = W + 1;
     const int line0 = blockIdx.x * W;
-    const int kz = line0 / (2 * ny), ky0 = line0 % (2 * ny);
+    const int kz = kz0 + line0 / (2 * ny), ky0 = line0 % (2 * ny);    // line0 counts within the slab
     const int tid = threadIdx.x, nt = blockDim.x;
     cplx *base = B + (size_t)line0 * nx;
     for (int idx = tid; idx < nx * W; idx += nt) {

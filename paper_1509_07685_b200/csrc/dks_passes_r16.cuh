@@ -22,6 +22,10 @@
 namespace dks {
 
 constexpr int kCols = 8;   // columns per CTA of the strided passes
+#ifndef DKS_R16_OCC
+#define DKS_R16_OCC 512
+#endif
+#define DKS_R16_MINB(A) (DKS_R16_OCC / R16Geom<A>::THREADS)
 
 template <int A>
 struct R16Geom {
@@ -74,17 +78,17 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
 // P2: forward y.  grid (nx / 8, nz + 1), 16 A threads.
 // ---------------------------------------------------------------------------------------------
 template <int A>
-__global__ void __launch_bounds__(R16Geom<A>::THREADS, 512 / R16Geom<A>::THREADS)
-p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d,
+__global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
+p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int kz0,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     extern __shared__ cplx ex[];
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
-    const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
+    const int nx = d.nx, ny = d.ny, kz = blockIdx.y;          // kz: plane within the slab
     const size_t x = (size_t)blockIdx.x * kCols + c;
     cplx v[16];
 #pragma unroll
-    for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)kz * ny + a + A * b) * nx + x]);
+    for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
     strided_forward<A>(v, ex, c, p, a, tw1, tw2);
 #pragma unroll
     for (int r = 0; r < 16; ++r)
@@ -95,8 +99,8 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d,
 // P4: inverse y, crop to ny.  grid (nx / 8, nz + 1)
 // ---------------------------------------------------------------------------------------------
 template <int A>
-__global__ void __launch_bounds__(R16Geom<A>::THREADS, 512 / R16Geom<A>::THREADS)
-p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d,
+__global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
+p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, int kz0,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     extern __shared__ cplx ex[];
@@ -112,7 +116,7 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d,
     combine_parities<8>(v, p, out);
 #pragma unroll
     for (int i = 0; i < 8; ++i)
-        stg_stream(&Aout[((size_t)kz * ny + a + A * (i + 8 * p)) * nx + x], out[i]);
+        stg_stream(&Aout[((size_t)(kz0 + kz) * ny + a + A * (i + 8 * p)) * nx + x], out[i]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -121,7 +125,7 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d,
 // grid (nx / 16, ny)
 // ---------------------------------------------------------------------------------------------
 template <int A>
-__global__ void __launch_bounds__(R16Geom<A>::THREADS, 512 / R16Geom<A>::THREADS)
+__global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
@@ -153,7 +157,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
 // C[L-k] = conj Fa[k] + i conj Fb[k] in shared memory first.  grid (nx / 16, ny)
 // ---------------------------------------------------------------------------------------------
 template <int A>
-__global__ void __launch_bounds__(R16Geom<A>::THREADS, 512 / R16Geom<A>::THREADS)
+__global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
@@ -214,7 +218,7 @@ constexpr int kP3SmemTw2 = 256 * (int)sizeof(cplx);
 constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp + kP3SmemTw2;
 
 __global__ void __launch_bounds__(kP3Warps * 32, 1)
-p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
+p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, int planes,
               const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -234,10 +238,10 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     }
     __syncthreads();
 
-    const unsigned ny2 = 2 * d.ny, nlines = (unsigned)(d.nz + 1) * ny2, stride = gridDim.x * kP3Warps;
+    const unsigned ny2 = 2 * d.ny, nlines = (unsigned)planes * ny2, stride = gridDim.x * kP3Warps;
     unsigned line = blockIdx.x * kP3Warps + warp;
     auto ghat_row = [&](unsigned l) {
-        const int kz = (int)(l / ny2), ky = (int)(l % ny2);
+        const int kz = kz0 + (int)(l / ny2), ky = (int)(l % ny2);
         return Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch;
     };
     if (lane == 0 && line < nlines) {

@@ -70,6 +70,12 @@ struct dks_poisson_plan {
     cplx *A = nullptr, *B = nullptr;
     double *G = nullptr, *stage = nullptr;
     size_t offA, offB, offG, offS, need_bytes;
+    // P2..P4 run slab by slab (slab = `slab` consecutive kz planes) so that B, the largest intermediate,
+    // is a slab-sized scratch that stays resident in L2 between the three passes
+    int slab = 0;                       // planes per slab, 1..nz+1
+    bool slab_user = false;             // set through dks_poisson_set_slab_planes
+    struct Step { int pass, kz0, planes; };
+    std::vector<Step> steps;            // the launch list of one solve
     bool greens_ready = false;
     bool setup_pending = false;         // setup_done not yet known to have completed
     cudaStream_t setup_stream = nullptr;
@@ -84,7 +90,7 @@ struct dks_poisson_plan {
 };
 
 static const int kNumPasses = 5;
-static const int kMaxProfSlots = 1024;
+static const int kMaxProfSlots = 256;
 
 static bool is_pow2_in_range(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
 static int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
@@ -98,15 +104,38 @@ static int tile_width_for(int L)
     return 4;
 }
 
+// Bytes of B the L2 is asked to keep between P2, P3 and P4 of one slab (B200: 126 MB of L2).
+static const size_t kSlabTargetBytes = (size_t)1 << 40;   // measured: slabbing loses, so automatic = one slab
+
+static int auto_slab(const dks_poisson_plan *p)
+{
+    const size_t plane = (size_t)16 * p->d.nx * 2 * p->d.ny;
+    const int planes = p->d.nz + 1;
+    int s = (int)std::max<size_t>(1, kSlabTargetBytes / plane);
+    if (s >= planes) return planes;
+    const int count = (planes + s - 1) / s;          // equalise the slabs
+    return (planes + count - 1) / count;
+}
+
+// [ A | Ghat | staging | B(slab) ]: B last, so that changing the slab size moves nothing else
 static void compute_layout(dks_poisson_plan *p)
 {
     const size_t nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
     size_t off = 0;
     p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1), 256);
-    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (nz + 1), 256);
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
     p->offS = off; off = align_up(off + 8 * nx * ny * nz, 256);
+    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)p->slab, 256);
     p->need_bytes = off;
+    p->steps.clear();
+    p->steps.push_back({ 1, 0, 0 });
+    for (int kz0 = 0; kz0 <= p->d.nz; kz0 += p->slab) {
+        const int planes = std::min(p->slab, p->d.nz + 1 - kz0);
+        p->steps.push_back({ 2, kz0, planes });
+        p->steps.push_back({ 3, kz0, planes });
+        p->steps.push_back({ 4, kz0, planes });
+    }
+    p->steps.push_back({ 5, 0, 0 });
 }
 
 static void bind_workspace(dks_poisson_plan *p)
@@ -173,6 +202,7 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_x = (size_t)2 * nx * (p->Wx + 1) * sizeof(cplx);
     p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
+    p->slab = auto_slab(p);
     compute_layout(p);
     g_err[0] = 0;
     return p;
@@ -224,32 +254,48 @@ static int r16_set_attributes()
 }
 
 template <int A>
-static void launch_strided_r16(int pass, const dks_poisson_plan *p, const double *rho, double *phi, cudaStream_t st)
+static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
+                               cudaStream_t st)
 {
     const MeshDims d = p->d;
     const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
-    switch (pass) {
+    switch (s.pass) {
     case 1: p1_z_r2c_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(rho, p->A, d, p->tw1[2], p->tw[2]); break;
-    case 2: p2_y_fwd_r16<A><<<dim3(d.nx / kCols, d.nz + 1), T, S, st>>>(p->A, p->B, d, p->tw1[1], p->tw[1]); break;
-    case 4: p4_y_inv_r16<A><<<dim3(d.nx / kCols, d.nz + 1), T, S, st>>>(p->B, p->A, d, p->tw1[1], p->tw[1]); break;
+    case 2: p2_y_fwd_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 4: p4_y_inv_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
     case 5: p5_z_c2r_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(p->A, phi, d, p->tw1[2], p->tw[2]); break;
     }
 }
 
-static void launch_r16(int pass, const dks_poisson_plan *p, const double *rho, double *phi, cudaStream_t st)
+static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
+                       cudaStream_t st)
 {
-    if (pass == 3) {
+    if (s.pass == 3) {
         const MeshDims d = p->d;
-        const unsigned lines = (unsigned)(d.nz + 1) * 2 * d.ny;
+        const unsigned lines = (unsigned)s.planes * 2 * d.ny;
         const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (lines + kP3Warps - 1) / kP3Warps);
-        p3_x_conv_r16<<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, p->tw1[0], p->tw[0]);
+        p3_x_conv_r16<<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, s.kz0, s.planes, p->tw1[0], p->tw[0]);
         return;
     }
-    const int A = (pass == 1 || pass == 5) ? p->r16A[2] : p->r16A[1];
+    const int A = (s.pass == 1 || s.pass == 5) ? p->r16A[2] : p->r16A[1];
     switch (A) {
-#define X(A_) case A_: launch_strided_r16<A_>(pass, p, rho, phi, st); break;
+#define X(A_) case A_: launch_strided_r16<A_>(s, p, rho, phi, st); break;
         DKS_FOR_EACH_A(X)
 #undef X
+    }
+}
+
+static void launch_generic(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
+                           cudaStream_t st)
+{
+    const MeshDims d = p->d;
+    switch (s.pass) {
+    case 1: p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]); break;
+    case 2: p2_y_fwd_generic<<<dim3(d.nx / p->Wy, s.planes), 256, p->smem_y, st>>>(p->A, p->B, d, s.kz0, p->Wy, p->tw[1]); break;
+    case 3: p3_x_conv_generic<<<(unsigned)((size_t)s.planes * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, s.kz0,
+                                                                                                    p->Wx, p->tw[0]); break;
+    case 4: p4_y_inv_generic<<<dim3(d.nx / p->Wy, s.planes), 256, p->smem_y, st>>>(p->B, p->A, d, s.kz0, p->Wy, p->tw[1]); break;
+    case 5: p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]); break;
     }
 }
 
@@ -314,6 +360,32 @@ extern "C" int dks_poisson_set_workspace(dks_poisson_plan *p, void *dev_ptr, siz
     bind_workspace(p);
     p->greens_ready = false;
     return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_slab_planes(dks_poisson_plan *p, int planes)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (planes < 0 || planes > p->d.nz + 1) return fail(DKS_ERR_INVALID_ARG, "planes must be in [0, nz+1] (0 = automatic)");
+    const int old = p->slab;
+    p->slab = planes ? planes : auto_slab(p);
+    compute_layout(p);
+    if (p->ws && p->ws_bytes < p->need_bytes) {
+        const size_t need = p->need_bytes;
+        p->slab = old;
+        compute_layout(p);
+        return fail(DKS_ERR_WORKSPACE_TOO_SMALL, "the attached workspace has %zu bytes, %zu needed for slabs of %d planes; "
+                    "set the slab size before attaching the workspace / before dks_greens_setup", p->ws_bytes, need, planes);
+    }
+    p->slab_user = planes != 0;
+    p->prof_slots = 0;                  // the launch list changed: recorded events no longer match
+    if (p->ws) bind_workspace(p);
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_slab_planes(const dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    return p->slab;
 }
 
 extern "C" int dks_poisson_set_stream(dks_poisson_plan *p, void *stream)
@@ -413,7 +485,7 @@ extern "C" int dks_poisson_copy_greens_hat(dks_poisson_plan *p, double *host_out
 extern "C" int dks_poisson_launches_per_solve(const dks_poisson_plan *p)
 {
     if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
-    return kNumPasses;
+    return (int)p->steps.size();
 }
 
 extern "C" double dks_poisson_model_bytes(const dks_poisson_plan *p, int pass)
@@ -442,6 +514,9 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     return p->fast[pass - 1] ? fast_names[pass - 1] : names[pass - 1];
 }
 
+// Events of one profiled solve: one before every launch of the launch list and one after the last.
+static size_t prof_stride(const dks_poisson_plan *p) { return p->steps.size() + 1; }
+
 extern "C" int dks_poisson_set_profiling(dks_poisson_plan *p, int slots)
 {
     if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
@@ -450,7 +525,7 @@ extern "C" int dks_poisson_set_profiling(dks_poisson_plan *p, int slots)
         int rc = ensure_device(p);
         if (rc) return rc;
     }
-    const size_t need = (size_t)slots * (kNumPasses + 1);
+    const size_t need = (size_t)slots * prof_stride(p);
     while (p->ev.size() < need) {
         cudaEvent_t e;
         DKS_CUDA(cudaEventCreate(&e));
@@ -467,14 +542,14 @@ extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int co
     if (p->prof_slots == 0 || p->prof_count == 0) return fail(DKS_ERR_NOT_SETUP, "no profiled solve has been issued");
     const int n = std::min(count, kNumPasses);
     const long long solves = std::min<long long>(p->prof_count, p->prof_slots);
-    std::vector<double> acc(n, 0.0);
+    std::vector<double> acc(kNumPasses, 0.0);
     for (long long s = 0; s < solves; ++s) {
-        cudaEvent_t *e = &p->ev[(size_t)s * (kNumPasses + 1)];
-        DKS_CUDA(cudaEventSynchronize(e[kNumPasses]));
-        for (int i = 0; i < n; ++i) {
+        cudaEvent_t *e = &p->ev[(size_t)s * prof_stride(p)];
+        DKS_CUDA(cudaEventSynchronize(e[p->steps.size()]));
+        for (size_t i = 0; i < p->steps.size(); ++i) {
             float ms = 0.f;
             DKS_CUDA(cudaEventElapsedTime(&ms, e[i], e[i + 1]));
-            acc[i] += ms;
+            acc[p->steps[i].pass - 1] += ms;
         }
     }
     for (int i = 0; i < n; ++i) ms_out[i] = (float)(acc[i] / (double)solves);
@@ -488,7 +563,6 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
         return fail(DKS_ERR_INVALID_ARG, "rho and phi must be 16-byte aligned");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const MeshDims d = p->d;
     if (p->setup_pending) {
         // Order this solve after the Green's setup.  A stream under capture must not wait on work
         // recorded outside the capture, so there the host waits for the setup instead (once).
@@ -508,24 +582,14 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
         }
     }
     const bool prof = p->prof_slots > 0;
-    cudaEvent_t *ev = prof ? &p->ev[(size_t)(p->prof_count % p->prof_slots) * (kNumPasses + 1)] : nullptr;
-    if (prof) DKS_CUDA(cudaEventRecord(ev[0], st));
-    if (p->fast[0]) launch_r16(1, p, rho, phi, st);
-    else p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]);
-    if (prof) DKS_CUDA(cudaEventRecord(ev[1], st));
-    if (p->fast[1]) launch_r16(2, p, rho, phi, st);
-    else p2_y_fwd_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->A, p->B, d, p->Wy, p->tw[1]);
-    if (prof) DKS_CUDA(cudaEventRecord(ev[2], st));
-    if (p->fast[2]) launch_r16(3, p, rho, phi, st);
-    else p3_x_conv_generic<<<(unsigned)((size_t)(d.nz + 1) * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, p->Wx,
-                                                                                                      p->tw[0]);
-    if (prof) DKS_CUDA(cudaEventRecord(ev[3], st));
-    if (p->fast[3]) launch_r16(4, p, rho, phi, st);
-    else p4_y_inv_generic<<<dim3(d.nx / p->Wy, d.nz + 1), 256, p->smem_y, st>>>(p->B, p->A, d, p->Wy, p->tw[1]);
-    if (prof) DKS_CUDA(cudaEventRecord(ev[4], st));
-    if (p->fast[4]) launch_r16(5, p, rho, phi, st);
-    else p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]);
-    if (prof) { DKS_CUDA(cudaEventRecord(ev[5], st)); ++p->prof_count; }
+    cudaEvent_t *ev = prof ? &p->ev[(size_t)(p->prof_count % p->prof_slots) * prof_stride(p)] : nullptr;
+    for (size_t i = 0; i < p->steps.size(); ++i) {
+        const dks_poisson_plan::Step &s = p->steps[i];
+        if (prof) DKS_CUDA(cudaEventRecord(ev[i], st));
+        if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, st);
+        else launch_generic(s, p, rho, phi, st);
+    }
+    if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
     DKS_CUDA(cudaGetLastError());
     return DKS_OK;
 }

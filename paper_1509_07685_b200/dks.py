@@ -34,6 +34,8 @@ SYMBOLS = {
     "dks_poisson_workspace_bytes": (_sz, [_vp]),
     "dks_poisson_set_workspace": (_i, [_vp, _vp, _sz]),
     "dks_poisson_set_stream": (_i, [_vp, _vp]),
+    "dks_poisson_set_slab_planes": (_i, [_vp, _i]),
+    "dks_poisson_slab_planes": (_i, [_vp]),
     "dks_poisson_set_profiling": (_i, [_vp, _i]),
     "dks_poisson_pass_times": (_i, [_vp, C.POINTER(C.c_float), _i]),
     "dks_poisson_launches_per_solve": (_i, [_vp]),
@@ -132,6 +134,14 @@ def dks_poisson_set_stream(plan, stream):
     return _check(lib.dks_poisson_set_stream(plan, stream), "dks_poisson_set_stream")
 
 
+def dks_poisson_set_slab_planes(plan, planes):
+    return _check(lib.dks_poisson_set_slab_planes(plan, int(planes)), "dks_poisson_set_slab_planes")
+
+
+def dks_poisson_slab_planes(plan) -> int:
+    return _check(lib.dks_poisson_slab_planes(plan), "dks_poisson_slab_planes")
+
+
 def dks_poisson_set_profiling(plan, slots):
     return _check(lib.dks_poisson_set_profiling(plan, int(slots)), "dks_poisson_set_profiling")
 
@@ -162,7 +172,7 @@ def dks_poisson_copy_greens_hat(plan, host_out):
 class PoissonPlan:
     """Owns a dks_poisson_plan and a torch-allocated workspace on the current CUDA device."""
 
-    def __init__(self, n, h, g0=None, own_workspace=True):
+    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None):
         import torch
 
         self.n, self.h = tuple(int(v) for v in n), tuple(float(v) for v in h)
@@ -170,6 +180,8 @@ class PoissonPlan:
         self._ws = None
         if g0 is not None:
             dks_poisson_set_g0(self._plan, g0)
+        if slab_planes is not None:
+            dks_poisson_set_slab_planes(self._plan, slab_planes)
         if own_workspace:
             nbytes = dks_poisson_workspace_bytes(self._plan)
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
