@@ -59,6 +59,22 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def max_over_ranks(ms_local: float, device="cpu") -> float:
+    """Device time of the slowest rank (replicas only: there is no data-path collective; this all-reduce of one
+    scalar is the measurement's own).  Works on NCCL (device="cuda") and on gloo (device="cpu")."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, ms_max: float) -> float:
+    """Solves/s of the whole job: every rank did `steps` solves of its own bunch in at most ms_max."""
+    return world * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
 
@@ -233,12 +249,9 @@ def run_ours(args):
         plan.solve(d_rho, d_phi)
     pass_ms = dks.dks_poisson_pass_times(plan.handle)
     dks.dks_poisson_set_profiling(plan.handle, 0)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if distributed:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, "cuda")
     ms_per_step = ms_total / args.steps
-    value = world * args.steps / (ms_total * 1e-3)
+    value = whole_job_value(world, args.steps, ms_total)
 
     # ---- end to end through the public API with HOST buffers (H2D + solve + D2H per step) --------
     h_rho = torch.from_numpy(rho).pin_memory()
@@ -251,10 +264,7 @@ def run_ours(args):
         plan.solve_host(h_rho, h_phi)
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if distributed:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * args.e2e_steps / (float(t.item()) * 1e-3)
+    e2e_value = whole_job_value(world, args.e2e_steps, max_over_ranks(e0.elapsed_time(e1), "cuda"))
 
     if rank != 0:
         plan.close()

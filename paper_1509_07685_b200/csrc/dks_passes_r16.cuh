@@ -122,8 +122,16 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
 // ---------------------------------------------------------------------------------------------
 // P1: forward z, real -> complex; the real columns (x, x+1) are packed into one complex line and
 // the packed spectrum C is split with FT{a}[k] = (C[k] + conj C[L-k]) / 2, FT{b}[k] = (C[k] - conj C[L-k]) / (2i).
-// grid (nx / 16, ny)
+// Persistent: CTA t, t + grid, ... over the (nx / 16) * ny tiles of 16 real columns.  The next tile's
+// rho rows (N rows x 128 B) arrive in the shared-memory stage through cp.async while this tile is
+// transformed, so the DRAM latency is never exposed.  Split output: 16 lanes store one 256-byte row.
 // ---------------------------------------------------------------------------------------------
+template <int A>
+struct P1Geom {
+    static constexpr int STAGE = 16 * A * kCols * (int)sizeof(cplx);     // N rows x 8 packed pairs
+    static constexpr int SMEM = R16Geom<A>::SMEM + STAGE;
+};
+
 template <int A>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d,
@@ -131,24 +139,54 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
 {
     extern __shared__ cplx ex[];
     constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
+    cplx *stage = ex + L * kCols;
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
-    const int nx = d.nx, ny = d.ny, y = blockIdx.y;
-    const size_t x0 = (size_t)blockIdx.x * 2 * kCols;
-    cplx v[16];
+    const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny;
+    auto prefetch = [&](int t) {
+        const int y = t / xtiles;
+        const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
 #pragma unroll
-    for (int b = 0; b < 16; ++b)
-        v[b] = ldg_stream(reinterpret_cast<const cplx *>(&rho[((size_t)(a + A * b) * ny + y) * nx + x0 + 2 * c]));
-    strided_forward<A>(v, ex, c, p, a, tw1, tw2);
-    __syncthreads();                                  // exchange reads done: reuse ex as C[K][c]
+        for (int i = 0; i < N * kCols / THREADS; ++i) {
+            const int idx = tid + i * THREADS, r = idx >> 3, cc = idx & 7;
+            cp_async16(&stage[idx], &rho[((size_t)r * ny + y) * nx + x0 + 2 * cc]);
+        }
+        cp_async_commit();
+    };
+    int t = blockIdx.x;
+    if (t < tiles) prefetch(t);
+    for (; t < tiles; t += gridDim.x) {
+        const int y = t / xtiles;
+        const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
+        cp_async_wait_all();
+        __syncthreads();                                  // stage complete; last tile's split reads done
+        cplx v[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) ex[(2 * (a + A * r) + p) * kCols + c] = v[r];
-    __syncthreads();
-    for (int idx = tid; idx < (N + 1) * kCols; idx += THREADS) {
-        const int k = idx >> 3, cc = idx & 7;
-        const cplx ck = ex[k * kCols + cc], cm = ex[((L - k) & (L - 1)) * kCols + cc];
-        cplx *out = &Aout[((size_t)k * ny + y) * nx + x0 + 2 * cc];
-        stg_stream(out, cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)));
-        stg_stream(out + 1, cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x)));
+        for (int b = 0; b < 16; ++b) v[b] = stage[(a + A * b) * kCols + c];
+        // ---- strided_forward, with the prefetch of the next tile issued once the stage is consumed
+        if (p) twiddle_parity<A, -1>(v, tw2, a);
+        fft16<-1>(v);
+        twiddle_between<A, -1>(v, tw1, a);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+        __syncthreads();
+        if (t + (int)gridDim.x < tiles) prefetch(t + gridDim.x);
+        constexpr int G = 16 / A;
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
+        fft_second<A, -1>(v);
+        __syncthreads();                                  // exchange reads done: reuse ex as C[K][c]
+#pragma unroll
+        for (int r = 0; r < 16; ++r) ex[(2 * (a + A * r) + p) * kCols + c] = v[r];
+        __syncthreads();
+        for (int idx = tid; idx < (N + 1) * 2 * kCols; idx += THREADS) {
+            const int k = idx >> 4, j = idx & 15, cc = j >> 1;
+            const cplx ck = ex[k * kCols + cc], cm = ex[((L - k) & (L - 1)) * kCols + cc];
+            const cplx o = (j & 1) ? cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x))
+                                   : cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y));
+            stg_stream(&Aout[((size_t)k * ny + y) * nx + x0 + j], o);
+        }
     }
 }
 

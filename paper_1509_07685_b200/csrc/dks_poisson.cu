@@ -243,7 +243,7 @@ extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
 static int r16_set_attributes()
 {
 #define X(A_)                                                                                                         \
-    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
@@ -260,7 +260,11 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
     const MeshDims d = p->d;
     const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
     switch (s.pass) {
-    case 1: p1_z_r2c_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(rho, p->A, d, p->tw1[2], p->tw[2]); break;
+    case 1: {
+        const int tiles = d.nx / (2 * kCols) * d.ny, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
+        p1_z_r2c_r16<A><<<std::min(tiles, p->sm_count * per_sm), T, P1Geom<A>::SMEM, st>>>(rho, p->A, d, p->tw1[2], p->tw[2]);
+        break;
+    }
     case 2: p2_y_fwd_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
     case 4: p4_y_inv_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
     case 5: p5_z_c2r_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(p->A, phi, d, p->tw1[2], p->tw[2]); break;
