@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -18,6 +19,7 @@
 #include "../../include/dks_poisson.h"
 #include "dks_passes_generic.cuh"
 #include "dks_passes_r16.cuh"
+#include "dks_fused_r16.cuh"
 
 using namespace dks;
 
@@ -74,7 +76,12 @@ struct dks_poisson_plan {
     // is a slab-sized scratch that stays resident in L2 between the three passes
     int slab = 0;                       // planes per slab, 1..nz+1
     bool slab_user = false;             // set through dks_poisson_set_slab_planes
-    struct Step { int pass, kz0, planes; };
+    struct Step { int pass, kz0, planes; };     // pass 1..5, or kPassFused = P2+P3+P4 of all planes in one kernel
+    // fused P2+P3+P4 (dks_fused_r16.cuh): available for nx = 256 and ny = 64, 128, 256
+    bool fused_ok = false, use_fused = false;
+    unsigned long long *dbg = nullptr;  // DKS_DEBUG: per-stage clock accumulators of the fused kernel
+    int fused_cl = 4;                   // CTAs per cluster
+    int fused_clusters = 0;             // clusters of kFusedCluster CTAs that are co-resident on this device
     std::vector<Step> steps;            // the launch list of one solve
     bool greens_ready = false;
     bool setup_pending = false;         // setup_done not yet known to have completed
@@ -90,6 +97,7 @@ struct dks_poisson_plan {
 };
 
 static const int kNumPasses = 5;
+static const int kPassFused = 6;
 static const int kMaxProfSlots = 256;
 
 static bool is_pow2_in_range(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
@@ -129,6 +137,11 @@ static void compute_layout(dks_poisson_plan *p)
     p->need_bytes = off;
     p->steps.clear();
     p->steps.push_back({ 1, 0, 0 });
+    if (p->use_fused) {
+        p->steps.push_back({ kPassFused, 0, p->d.nz + 1 });
+        p->steps.push_back({ 5, 0, 0 });
+        return;
+    }
     for (int kz0 = 0; kz0 <= p->d.nz; kz0 += p->slab) {
         const int planes = std::min(p->slab, p->d.nz + 1 - kz0);
         p->steps.push_back({ 2, kz0, planes });
@@ -203,6 +216,8 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
     p->slab = auto_slab(p);
+    p->fused_ok = p->fast[1] && p->fast[2] && p->r16A[1] >= 4;
+    p->use_fused = false;               // measured slower than the separate passes so far: opt-in
     compute_layout(p);
     g_err[0] = 0;
     return p;
@@ -231,6 +246,15 @@ static void release_device(dks_poisson_plan *p)
 extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
 {
     if (!p) return;
+    if (p->dbg) {
+        unsigned long long h[6];
+        if (cudaMemcpy(h, p->dbg, sizeof(h), cudaMemcpyDeviceToHost) == cudaSuccess) {
+            double tot = 0; for (int i = 0; i < 6; ++i) tot += (double)h[i];
+            fprintf(stderr, "dks: fused stage clocks S1 %.1f%% bar %.1f%% | S2 %.1f%% bar %.1f%% | S3 %.1f%% bar %.1f%%\n", 100 * h[0] / tot,
+                    100 * h[1] / tot, 100 * h[2] / tot, 100 * h[3] / tot, 100 * h[4] / tot, 100 * h[5] / tot);
+        }
+        cudaFree(p->dbg);
+    }
     release_device(p);
     delete p;
 }
@@ -252,6 +276,48 @@ static int r16_set_attributes()
     DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem));
     return DKS_OK;
 }
+
+template <int A, int CL>
+static int fused_prepare(dks_poisson_plan *p)
+{
+    DKS_CUDA(cudaFuncSetAttribute(p234_fused_r16<A, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFusedSmem));
+    if (CL > 8) DKS_CUDA(cudaFuncSetAttribute(p234_fused_r16<A, CL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(CL * 64); cfg.blockDim = dim3(kFusedThreads); cfg.dynamicSmemBytes = kFusedSmem;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    int n = 0;
+    DKS_CUDA(cudaOccupancyMaxActiveClusters(&n, p234_fused_r16<A, CL>, &cfg));
+    p->fused_clusters = n;
+    if (getenv("DKS_DEBUG")) {
+        fprintf(stderr, "dks: fused A=%d: %d co-resident clusters of %d CTAs\n", A, n, CL);
+        if (getenv("DKS_STAGE_CLOCKS") && !p->dbg) {
+            DKS_CUDA(cudaMalloc(&p->dbg, 6 * sizeof(unsigned long long)));
+            DKS_CUDA(cudaMemset(p->dbg, 0, 6 * sizeof(unsigned long long)));
+        }
+    }
+    return DKS_OK;
+}
+
+template <int A, int CL>
+static int fused_launch(const dks_poisson_plan *p, cudaStream_t st)
+{
+    const int clusters = std::min(p->fused_clusters, std::min(p->d.nz + 1, p->slab));   // B holds `slab` planes
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(CL * clusters); cfg.blockDim = dim3(kFusedThreads); cfg.dynamicSmemBytes = kFusedSmem;
+    cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
+    DKS_CUDA(cudaLaunchKernelEx(&cfg, p234_fused_r16<A, CL>, p->A, p->B, (const double *)p->G, p->d, (const cplx *)p->tw1[0],
+                                (const cplx *)p->tw[0], (const cplx *)p->tw1[1], (const cplx *)p->tw[1], p->dbg, getenv("DKS_FUSED_SKIP") ? atoi(getenv("DKS_FUSED_SKIP")) : 0));
+    return DKS_OK;
+}
+
+// (A, cluster size) instantiations
+#define DKS_FOR_EACH_FUSED(X) X(4, 4) X(8, 4) X(16, 4) X(4, 8) X(8, 8) X(16, 8) X(16, 2) X(16, 16)
 
 template <int A>
 static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
@@ -343,6 +409,17 @@ static int ensure_device(dks_poisson_plan *p)
     DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g));
     int rc = r16_set_attributes();
     if (rc) return rc;
+    if (p->fused_ok) {
+        if (const char *e = getenv("DKS_FUSED_CL")) p->fused_cl = atoi(e);
+#define X(A_, CL_) if (p->r16A[1] == A_ && p->fused_cl == CL_) rc = fused_prepare<A_, CL_>(p);
+        DKS_FOR_EACH_FUSED(X)
+#undef X
+        if (rc) return rc;
+        if (p->fused_clusters < 1) {         // no co-resident cluster on this device: fall back to separate passes
+            p->fused_ok = p->use_fused = false;
+            compute_layout(p);
+        }
+    }
     p->device_checked = true;
     return DKS_OK;
 }
@@ -384,6 +461,22 @@ extern "C" int dks_poisson_set_slab_planes(dks_poisson_plan *p, int planes)
     p->prof_slots = 0;                  // the launch list changed: recorded events no longer match
     if (p->ws) bind_workspace(p);
     return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_fused(dks_poisson_plan *p, int on)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (on && !p->fused_ok) return fail(DKS_ERR_INVALID_ARG, "the fused P2+P3+P4 kernel needs nx = 256 and ny in {64, 128, 256}");
+    p->use_fused = on != 0;
+    p->prof_slots = 0;
+    compute_layout(p);
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_fused(const dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    return p->use_fused ? 1 : 0;
 }
 
 extern "C" int dks_poisson_slab_planes(const dks_poisson_plan *p)
@@ -498,6 +591,7 @@ extern "C" double dks_poisson_model_bytes(const dks_poisson_plan *p, int pass)
     const double nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
     const double rho = 8 * nx * ny * nz, a = 16 * nx * ny * (nz + 1), b = 2 * a;
     const double g = 8 * (nx + 1) * (ny + 1) * (nz + 1);
+    if (p->use_fused && pass >= 2 && pass <= 4) return pass == 3 ? 2 * a + g : 0.0;   // B stays in L2
     switch (pass) {
     case 0: return 2 * rho + 4 * a + 4 * b + g;
     case 1: return rho + a;
@@ -515,6 +609,7 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     static const char *names[5] = { "p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic",
                                     "p4_y_inv_generic", "p5_z_c2r_generic" };
     static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
+    if (p->use_fused && pass >= 2 && pass <= 4) return pass == 3 ? "p234_fused_r16" : "(fused into p234_fused_r16)";
     return p->fast[pass - 1] ? fast_names[pass - 1] : names[pass - 1];
 }
 
@@ -553,7 +648,7 @@ extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int co
         for (size_t i = 0; i < p->steps.size(); ++i) {
             float ms = 0.f;
             DKS_CUDA(cudaEventElapsedTime(&ms, e[i], e[i + 1]));
-            acc[p->steps[i].pass - 1] += ms;
+            acc[(p->steps[i].pass == kPassFused ? 3 : p->steps[i].pass) - 1] += ms;
         }
     }
     for (int i = 0; i < n; ++i) ms_out[i] = (float)(acc[i] / (double)solves);
@@ -590,7 +685,13 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
     for (size_t i = 0; i < p->steps.size(); ++i) {
         const dks_poisson_plan::Step &s = p->steps[i];
         if (prof) DKS_CUDA(cudaEventRecord(ev[i], st));
-        if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, st);
+        if (s.pass == kPassFused) {
+            int rc = DKS_OK;
+#define X(A_, CL_) if (p->r16A[1] == A_ && p->fused_cl == CL_) rc = fused_launch<A_, CL_>(p, st);
+            DKS_FOR_EACH_FUSED(X)
+#undef X
+            if (rc) return rc;
+        } else if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, st);
         else launch_generic(s, p, rho, phi, st);
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
