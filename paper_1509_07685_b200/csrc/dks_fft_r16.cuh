@@ -143,26 +143,60 @@ __device__ __forceinline__ void fft_second(cplx (&v)[16])
     for (int r = 0; r < 16; ++r) v[r] = o[r];
 }
 
-// twiddle between the two steps: v[k] *= w_n^(a k), table tw1[k A + a] = exp(-2 pi i a k / n)
+// Twiddle between the two steps: v[k] *= T[k A + a] (SIGN < 0) or conj(T[k A + a]) (SIGN > 0), k = 0..15.
+// T is one of the three n-entry regions of the per-axis table tw1 (host: build_tw1 in dks_poisson.cu):
+//   [0, n)    parity 0, both directions:  w_n^(a k)
+//   [n, 2n)   parity 1, forward:          w_n^(a k) w_L^a          (L = 2n)
+//   [2n, 3n)  parity 1, inverse:          w_n^(a k) w_L^(k mod A)
+// The parity-1 regions carry the thread-constant part of the parity twiddle w_L^(+-m), m = a + A b =
+// thread part + A * register part; the register part w_32^b is a compile-time constant (parity_consts).
+// So the parity twiddle costs no table access at all.  (Region 0 has T = 1 at k = 0.)
 template <int A, int SIGN>
-__device__ __forceinline__ void twiddle_between(cplx (&v)[16], const cplx *__restrict__ tw1, int a)
+__device__ __forceinline__ void twiddle_between(cplx (&v)[16], const cplx *__restrict__ T, int a)
 {
 #pragma unroll
-    for (int k = 1; k < 16; ++k) {
-        cplx t = __ldg(&tw1[k * A + a]);
+    for (int k = 0; k < 16; ++k) {
+        cplx t = __ldg(&T[k * A + a]);
         v[k] = SIGN < 0 ? cmul(v[k], t) : cmulc(v[k], t);
     }
 }
-
-// parity twiddle: v[b] *= w_L^(SIGN' (a + A b)); tw2[m] = exp(-2 pi i m / L), m < n
+// same, table in shared memory
 template <int A, int SIGN>
-__device__ __forceinline__ void twiddle_parity(cplx (&v)[16], const cplx *__restrict__ tw2, int a)
+__device__ __forceinline__ void twiddle_between_s(cplx (&v)[16], const cplx *T, int a)
 {
 #pragma unroll
-    for (int b = 0; b < 16; ++b) {
-        cplx t = __ldg(&tw2[a + A * b]);
-        v[b] = SIGN < 0 ? cmul(v[b], t) : cmulc(v[b], t);
-    }
+    for (int k = 0; k < 16; ++k) v[k] = SIGN < 0 ? cmul(v[k], T[k * A + a]) : cmulc(v[k], T[k * A + a]);
+}
+
+// cos, sin of 2 pi m / 32, m = 0..15
+__device__ __forceinline__ constexpr double cos32(int m)
+{
+    return m == 0 ? 1.0 : m == 1 ? 0.98078528040323044913 : m == 2 ? 0.92387953251128675613
+         : m == 3 ? 0.83146961230254523708 : m == 4 ? 0.70710678118654752440 : m == 5 ? 0.55557023301960222474
+         : m == 6 ? 0.38268343236508977173 : m == 7 ? 0.19509032201612826785 : m == 8 ? 0.0
+         : -cos32(16 - m);
+}
+__device__ __forceinline__ constexpr double sin32(int m) { return m <= 8 ? cos32(8 - m) : cos32(m - 8); }
+
+// a * exp(SIGN 2 pi i M / 32), M = 0..15 a compile-time constant
+template <int SIGN, int M>
+__device__ __forceinline__ cplx mul_w32(cplx a)
+{
+    if (M == 0) return a;
+    if (M == 8) return mul_si<SIGN>(a);
+    constexpr double c = cos32(M), s = SIGN * sin32(M);
+    return cmake(fma(a.x, c, -(a.y * s)), fma(a.x, s, a.y * c));
+}
+
+// register part of the parity twiddle: v[b] *= exp(SIGN 2 pi i b / 32) = w_L^(-SIGN A b)
+template <int SIGN>
+__device__ __forceinline__ void parity_consts(cplx (&v)[16])
+{
+    v[1] = mul_w32<SIGN, 1>(v[1]);   v[2] = mul_w32<SIGN, 2>(v[2]);   v[3] = mul_w32<SIGN, 3>(v[3]);
+    v[4] = mul_w32<SIGN, 4>(v[4]);   v[5] = mul_w32<SIGN, 5>(v[5]);   v[6] = mul_w32<SIGN, 6>(v[6]);
+    v[7] = mul_w32<SIGN, 7>(v[7]);   v[8] = mul_w32<SIGN, 8>(v[8]);   v[9] = mul_w32<SIGN, 9>(v[9]);
+    v[10] = mul_w32<SIGN, 10>(v[10]); v[11] = mul_w32<SIGN, 11>(v[11]); v[12] = mul_w32<SIGN, 12>(v[12]);
+    v[13] = mul_w32<SIGN, 13>(v[13]); v[14] = mul_w32<SIGN, 14>(v[14]); v[15] = mul_w32<SIGN, 15>(v[15]);
 }
 
 __device__ __forceinline__ cplx shfl_xor_c(cplx v, int mask)

@@ -30,67 +30,43 @@ constexpr int kFusedWarps = kFusedThreads / 32;
 constexpr int kFusedNx = 256;                      // the line stage is written for nx = 256 (A_x = 16)
 
 // shared-memory layout (bytes)
-constexpr int kFusedOffTw1x = 0;                                   // [16][16] w_256^(a k)
-constexpr int kFusedOffTw2x = kFusedOffTw1x + 256 * 16;            // [256]    w_512^m
-constexpr int kFusedOffTw1y = kFusedOffTw2x + 256 * 16;            // [16][A]  w_n^(a k)      (n <= 256)
-constexpr int kFusedOffTw2y = kFusedOffTw1y + 256 * 16;            // [n]      w_2n^m
-constexpr int kFusedOffWork = kFusedOffTw2y + 256 * 16;            // union: team exchange buffers / per-warp line buffers
+constexpr int kFusedOffTw1x = 0;                                   // regions 0, 1 of the x table (twiddle_between): 2 x 256
+constexpr int kFusedOffTw1y = kFusedOffTw1x + 512 * 16;            // regions 0, 1, 2 of the y table: 3 x n, n <= 256
+constexpr int kFusedOffWork = kFusedOffTw1y + 768 * 16;            // union: team exchange buffers / per-warp line buffers
 constexpr int kFusedLineEx = 8192;                                 // per warp: exchange [2][16][16] cplx
 constexpr int kFusedLineG = 2112;                                  // per warp: Ghat row, 264 doubles
 constexpr int kFusedLineBytes = kFusedLineEx + kFusedLineG;        // 10304
 constexpr int kFusedWorkBytes = kFusedWarps * kFusedLineBytes;     // 164864 >= 2 teams x 64 KB
 constexpr int kFusedSmem = kFusedOffWork + kFusedWorkBytes;        // 181248
 
-// L2 eviction policies: the scratch plane must stay in L2 (evict_last); A and Ghat stream through once
-// (evict_first), so that they do not push the scratch out.
-__device__ __forceinline__ uint64_t l2_policy_evict_last()
-{
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first()
-{
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-// scratch read: another SM wrote the data, so L1 must not serve it (nothing ever allocates these lines in L1)
-__device__ __forceinline__ cplx ldg_scr(const cplx *p, uint64_t pol)
+// Scratch accesses: another SM wrote the data, so L1 must not serve it (ld.global.cg; nothing ever allocates
+// these lines in L1); the A plane and the Ghat rows stream through with L1::no_allocate.  (L2 eviction
+// policies through createpolicy / L2::cache_hint -- evict_last for the scratch, evict_first for the streams --
+// cut the scratch write-back traffic by a third but are left out: see DESIGN.md section 5.)
+__device__ __forceinline__ cplx ldg_scr(const cplx *p, uint64_t)
 {
     cplx r;
-    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
-                 : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol) : "memory");
+    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p) : "memory");
     return r;
 }
-__device__ __forceinline__ void stg_scr(cplx *p, cplx v, uint64_t pol)
+__device__ __forceinline__ void stg_scr(cplx *p, cplx v, uint64_t)
 {
-    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+    asm volatile("st.global.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
-__device__ __forceinline__ cplx ldg_once(const cplx *p, uint64_t pol)
-{
-    cplx r;
-    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;"
-                 : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
-    return r;
-}
-__device__ __forceinline__ void stg_once(cplx *p, cplx v, uint64_t pol)
-{
-    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol)
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async16_hint(void *smem_dst, const void *gmem_src, uint64_t pol)
-{
-    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "l"(pol)
-                 : "memory");
-}
-__device__ __forceinline__ void team_sync(int id, int count)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
-}
+__device__ __forceinline__ cplx ldg_once(const cplx *p, uint64_t) { return ldg_stream(p); }
+__device__ __forceinline__ void stg_once(cplx *p, cplx v, uint64_t) { stg_stream(p, v); }
+__device__ __forceinline__ void cp_async16_hint(void *smem_dst, const void *gmem_src, uint64_t) { cp_async16(smem_dst, gmem_src); }
+__device__ __forceinline__ uint64_t l2_policy_evict_last() { return 0; }
+__device__ __forceinline__ uint64_t l2_policy_evict_first() { return 0; }
+// The column-tile teams of a CTA run in lockstep behind __syncthreads(): every team has the same number of
+// tiles (the host only selects a cluster size with (nx / 8) % (CL * teams) == 0).  Named barriers per team
+// (bar.sync id, count) were tried first and produced sporadic cudaErrorIllegalInstruction on some
+// instantiations, depending on unrelated code changes; barrier 0 has never shown it.
+__device__ __forceinline__ void team_sync(int, int) { __syncthreads(); }
 __device__ __forceinline__ void cluster_sync_all()
 {
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    __cluster_barrier_arrive();        // release
+    __cluster_barrier_wait();          // acquire
 }
 __device__ __forceinline__ unsigned cluster_ctarank()
 {
@@ -120,7 +96,7 @@ __device__ __forceinline__ void cp_async_wait_all_fused() { asm volatile("cp.asy
 // ---- S1: this team's column tiles t0, t0 + tstep, ... < xtiles, forward y (arithmetic of p2_y_fwd_r16) --
 template <int A>
 __device__ __forceinline__ void fused_tiles_fwd(const cplx *__restrict__ Aplane, cplx *__restrict__ Bs, int nx, int t0, int tstep,
-                                                int xtiles, int tt, cplx *ex, const cplx *tw1s, const cplx *tw2s, int bar_id,
+                                                int xtiles, int tt, cplx *ex, const cplx *tw1s, int bar_id,
                                                 uint64_t keep, uint64_t once)
 {
     constexpr int T = 16 * A, G = 16 / A, N = 16 * A;
@@ -142,13 +118,9 @@ __device__ __forceinline__ void fused_tiles_fwd(const cplx *__restrict__ Aplane,
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = ex[(a + A * b) * kCols + c];
         team_sync(bar_id, T);                          // tile consumed: ex becomes the exchange buffer
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmul(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<-1>(v);
         fft16<-1>(v);
-#pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tw1s[k * A + a]);
+        twiddle_between_s<A, -1>(v, tw1s + p * N, a);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
         team_sync(bar_id, T);
@@ -167,7 +139,7 @@ __device__ __forceinline__ void fused_tiles_fwd(const cplx *__restrict__ Aplane,
 // ---- S3: this team's column tiles, inverse y + crop (arithmetic of p4_y_inv_r16) ----------------------
 template <int A>
 __device__ __forceinline__ void fused_tiles_inv(const cplx *__restrict__ Bs, cplx *__restrict__ Aplane, int nx, int t0, int tstep,
-                                                int xtiles, int tt, cplx *ex, const cplx *tw1s, const cplx *tw2s, int bar_id,
+                                                int xtiles, int tt, cplx *ex, const cplx *tw1s, int bar_id,
                                                 uint64_t keep, uint64_t once)
 {
     constexpr int T = 16 * A, G = 16 / A, N = 16 * A;
@@ -190,8 +162,7 @@ __device__ __forceinline__ void fused_tiles_inv(const cplx *__restrict__ Bs, cpl
         for (int b = 0; b < 16; ++b) v[b] = ex[(2 * (a + A * b) + p) * kCols + c];
         team_sync(bar_id, T);
         fft16<+1>(v);
-#pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tw1s[k * A + a]);
+        twiddle_between_s<A, +1>(v, tw1s + p * 2 * N, a);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
         team_sync(bar_id, T);
@@ -202,10 +173,7 @@ __device__ __forceinline__ void fused_tiles_inv(const cplx *__restrict__ Bs, cpl
         team_sync(bar_id, T);
         if (t + tstep < xtiles) prefetch(t + tstep);
         fft_second<A, +1>(v);
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmulc(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<+1>(v);
         cplx out[8];
         combine_parities<8>(v, p, out);
 #pragma unroll
@@ -218,7 +186,7 @@ __device__ __forceinline__ void fused_tiles_inv(const cplx *__restrict__ Bs, cpl
 // [2][16][16] (its first 4 KB double as the landing zone of the next line); gs: the warp's Ghat row.
 __device__ __forceinline__ void fused_lines(cplx *__restrict__ Bs, const double *__restrict__ Gplane, int gpitch, int nx, int ny2,
                                             int ky0, int kstep, int lane, cplx *exw, double *gs, const cplx *tw1s,
-                                            const cplx *tw2s, uint64_t keep, uint64_t once)
+                                            uint64_t keep, uint64_t once)
 {
     constexpr int A = 16, L = 512, N = 256;
     const int a = lane & 15, p = lane >> 4;
@@ -251,13 +219,9 @@ __device__ __forceinline__ void fused_lines(cplx *__restrict__ Bs, const double 
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = exw[a + A * b];
         __syncwarp();                                  // line consumed: exw becomes the exchange buffer
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmul(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<-1>(v);
         fft16<-1>(v);
-#pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tw1s[k * A + a]);
+        twiddle_between_s<A, -1>(v, tw1s + p * N, a);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
         __syncwarp();
@@ -271,9 +235,7 @@ __device__ __forceinline__ void fused_lines(cplx *__restrict__ Bs, const double 
         }
         __syncwarp();                                  // Ghat row consumed; forward exchange reads done
         if (more) prefetch_ghat(ky + kstep);
-        fft16<+1>(v);
-#pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tw1s[k * A + a]);
+        fft16<+1>(v);                                  // transposed inverse flow (see p3_x_conv_r16)
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
         __syncwarp();
@@ -281,11 +243,9 @@ __device__ __forceinline__ void fused_lines(cplx *__restrict__ Bs, const double 
         for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * 16 + (ap ^ (a & 7))];
         __syncwarp();                                  // exchange read by all lanes: exw free for the next line
         if (more) prefetch_line(ky + kstep);
+        twiddle_between_s<A, +1>(v, tw1s + p * N, a);
         fft16<+1>(v);
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmulc(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<+1>(v);
         cplx out[8];
         combine_parities<16>(v, p, out);
 #pragma unroll
@@ -300,26 +260,17 @@ __device__ __forceinline__ void fused_lines(cplx *__restrict__ Bs, const double 
 template <int A, int CL>
 __global__ void __launch_bounds__(kFusedThreads, 1)
 p234_fused_r16(cplx *__restrict__ Abuf, cplx *__restrict__ Bscr, const double *__restrict__ Ghat, MeshDims d,
-               const cplx *__restrict__ tw1x, const cplx *__restrict__ tw2x,
-               const cplx *__restrict__ tw1y, const cplx *__restrict__ tw2y, unsigned long long *dbg, int skip)
+               const cplx *__restrict__ tw1x, const cplx *__restrict__ tw1y)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    long long tacc[6] = { 0, 0, 0, 0, 0, 0 }, tprev = clock64();
-#define DKS_TICK(i) do { if (dbg) { long long now_ = clock64(); tacc[i] += now_ - tprev; tprev = now_; } } while (0)
     constexpr int T = 16 * A, TEAMS = kFusedThreads / T, N = 16 * A;
     cplx *tw1xs = reinterpret_cast<cplx *>(smem_raw + kFusedOffTw1x);
-    cplx *tw2xs = reinterpret_cast<cplx *>(smem_raw + kFusedOffTw2x);
     cplx *tw1ys = reinterpret_cast<cplx *>(smem_raw + kFusedOffTw1y);
-    cplx *tw2ys = reinterpret_cast<cplx *>(smem_raw + kFusedOffTw2y);
     unsigned char *work = smem_raw + kFusedOffWork;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int i = tid; i < 256; i += kFusedThreads) {
-        tw1xs[i] = __ldg(&tw1x[i]);
-        tw2xs[i] = __ldg(&tw2x[i]);
-        if (i < N) {
-            tw1ys[i] = __ldg(&tw1y[i]);
-            tw2ys[i] = __ldg(&tw2y[i]);
-        }
+    for (int i = tid; i < 768; i += kFusedThreads) {
+        if (i < 512) tw1xs[i] = __ldg(&tw1x[i]);
+        if (i < 3 * N) tw1ys[i] = __ldg(&tw1y[i]);
     }
     __syncthreads();
 
@@ -337,26 +288,17 @@ p234_fused_r16(cplx *__restrict__ Abuf, cplx *__restrict__ Bscr, const double *_
 
     for (int kz = cid; kz <= d.nz; kz += ncl) {
         cplx *Aplane = Abuf + (size_t)kz * ny * nx;
-        if (!(skip & 1)) fused_tiles_fwd<A>(Aplane, Bs, nx, rank * TEAMS + team, CL * TEAMS, xtiles, tt, ex_team, tw1ys, tw2ys, 1 + team, keep, once);
+        fused_tiles_fwd<A>(Aplane, Bs, nx, rank * TEAMS + team, CL * TEAMS, xtiles, tt, ex_team, tw1ys, 1 + team, keep, once);
         __syncthreads();
-        DKS_TICK(0);
         cluster_sync_all();
-        DKS_TICK(1);
-        if (!(skip & 2)) fused_lines(Bs, Ghat + (size_t)kz * (ny + 1) * d.gpitch, d.gpitch, nx, ny2, rank * kFusedWarps + warp, CL * kFusedWarps,
-                    lane, ex_warp, gs_warp, tw1xs, tw2xs, keep, once);
+        fused_lines(Bs, Ghat + (size_t)kz * (ny + 1) * d.gpitch, d.gpitch, nx, ny2, rank * kFusedWarps + warp, CL * kFusedWarps,
+                    lane, ex_warp, gs_warp, tw1xs, keep, once);
         __syncthreads();
-        DKS_TICK(2);
         cluster_sync_all();
-        DKS_TICK(3);
-        if (!(skip & 4)) fused_tiles_inv<A>(Bs, Aplane, nx, rank * TEAMS + team, CL * TEAMS, xtiles, tt, ex_team, tw1ys, tw2ys, 1 + team, keep, once);
+        fused_tiles_inv<A>(Bs, Aplane, nx, rank * TEAMS + team, CL * TEAMS, xtiles, tt, ex_team, tw1ys, 1 + team, keep, once);
         __syncthreads();
-        DKS_TICK(4);
         cluster_sync_all();
-        DKS_TICK(5);
     }
-    if (dbg && tid == 0)
-        for (int i = 0; i < 6; ++i) atomicAdd(&dbg[i], (unsigned long long)tacc[i]);
-#undef DKS_TICK
 }
 
 }  // namespace dks

@@ -41,9 +41,9 @@ template <int A>
 __device__ __forceinline__ void strided_forward(cplx (&v)[16], cplx *ex, int c, int p, int a,
                                                 const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
-    if (p) twiddle_parity<A, -1>(v, tw2, a);
+    if (p) parity_consts<-1>(v);
     fft16<-1>(v);
-    twiddle_between<A, -1>(v, tw1, a);
+    twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
     __syncthreads();
@@ -61,7 +61,7 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
                                                 const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     fft16<+1>(v);
-    twiddle_between<A, +1>(v, tw1, a);
+    twiddle_between<A, +1>(v, tw1 + p * 32 * A, a);
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
     __syncthreads();
@@ -71,7 +71,7 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
     fft_second<A, +1>(v);
-    if (p) twiddle_parity<A, +1>(v, tw2, a);
+    if (p) parity_consts<+1>(v);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -163,9 +163,9 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[(a + A * b) * kCols + c];
         // ---- strided_forward, with the prefetch of the next tile issued once the stage is consumed
-        if (p) twiddle_parity<A, -1>(v, tw2, a);
+        if (p) parity_consts<-1>(v);
         fft16<-1>(v);
-        twiddle_between<A, -1>(v, tw1, a);
+        twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
         __syncthreads();
@@ -252,8 +252,7 @@ constexpr int kP3OffEx = 4096;                     // after the 256-element line
 constexpr int kP3OffG = kP3OffEx + 8192;
 constexpr int kP3OffBar = kP3OffG + kP3GhatBytes;
 constexpr int kP3SmemPerWarp = kP3OffBar + 16;     // 14368
-constexpr int kP3SmemTw2 = 256 * (int)sizeof(cplx);
-constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp + kP3SmemTw2;
+constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp;
 
 __global__ void __launch_bounds__(kP3Warps * 32, 1)
 p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, int planes,
@@ -267,8 +266,6 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + p * 256;
     const double *gs = reinterpret_cast<const double *>(wb + kP3OffG);
     uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] line data, [1] Ghat row
-    cplx *tw2s = reinterpret_cast<cplx *>(smem_raw + kP3Warps * kP3SmemPerWarp);
-    for (int i = threadIdx.x; i < 256; i += kP3Warps * 32) tw2s[i] = __ldg(&tw2[i]);
     if (lane == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
@@ -288,10 +285,14 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
         mbar_expect_tx(&bar[1], kP3GhatBytes);
         bulk_g2s(wb + kP3OffG, ghat_row(line), kP3GhatBytes, &bar[1]);
     }
-    // between-step twiddles w_256^(a k), k = 1..15, fixed per lane
-    cplx tb[15];
+    // Between-step twiddles, fixed per lane: tb[k] = w_256^(a k) for parity 0, w_256^(a k) w_512^a for parity 1
+    // (regions 0 and 1 of tw1, see twiddle_between).  The inverse runs the TRANSPOSED flow (radix-16,
+    // exchange, twiddle, radix-16), in which the same per-lane set applies conjugated, so one register
+    // set serves both directions and the parity twiddle w_512^(+-m) needs no table: its lane part is in
+    // tb, its register part w_32^b is a compile-time constant (parity_consts).
+    cplx tb[16];
 #pragma unroll
-    for (int k = 1; k < 16; ++k) tb[k - 1] = __ldg(&tw1[k * A + a]);
+    for (int k = 0; k < 16; ++k) tb[k] = __ldg(&tw1[p * N + k * A + a]);
 
     unsigned phase = 0;
     for (; line < nlines; line += stride, phase ^= 1) {
@@ -307,13 +308,10 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             bulk_g2s(wb, B + (size_t)next * N, N * sizeof(cplx), &bar[0]);
         }
         // forward
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmul(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<-1>(v);
         fft16<-1>(v);
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tb[k - 1]);
+        for (int k = 0; k < 16; ++k) v[k] = cmul(v[k], tb[k]);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
         __syncwarp();
@@ -332,20 +330,15 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             mbar_expect_tx(&bar[1], kP3GhatBytes);
             bulk_g2s(wb + kP3OffG, ghat_row(next), kP3GhatBytes, &bar[1]);
         }
-        // inverse
+        // inverse, transposed flow: v[r] = X[2 (a + 16 r) + p] -> radix-16 over r -> exchange -> conj tb -> radix-16
         fft16<+1>(v);
-#pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tb[k - 1]);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
         __syncwarp();
 #pragma unroll
-        for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * 16 + (ap ^ (a & 7))];
+        for (int ap = 0; ap < 16; ++ap) v[ap] = cmulc(ex[a * 16 + (ap ^ (a & 7))], tb[ap]);
         fft16<+1>(v);
-        if (p) {
-#pragma unroll
-            for (int b = 0; b < 16; ++b) v[b] = cmulc(v[b], tw2s[a + A * b]);
-        }
+        if (p) parity_consts<+1>(v);
         cplx out[8];
         combine_parities<16>(v, p, out);
 #pragma unroll

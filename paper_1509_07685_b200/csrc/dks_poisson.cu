@@ -79,7 +79,6 @@ struct dks_poisson_plan {
     struct Step { int pass, kz0, planes; };     // pass 1..5, or kPassFused = P2+P3+P4 of all planes in one kernel
     // fused P2+P3+P4 (dks_fused_r16.cuh): available for nx = 256 and ny = 64, 128, 256
     bool fused_ok = false, use_fused = false;
-    unsigned long long *dbg = nullptr;  // DKS_DEBUG: per-stage clock accumulators of the fused kernel
     int fused_cl = 4;                   // CTAs per cluster
     int fused_clusters = 0;             // clusters of kFusedCluster CTAs that are co-resident on this device
     std::vector<Step> steps;            // the launch list of one solve
@@ -193,15 +192,21 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     for (int a = 0; a < 3; ++a) {
         const int n = ns[a];
         if (n < 32 || n > 256) continue;
-        const int A = n / 16;
+        const int A = n / 16, L = 2 * n;
         p->r16A[a] = A;
-        p->tw1_host[a].resize(n);
+        // three regions of n entries (dks_fft_r16.cuh, twiddle_between): exp(-2 pi i e / L) with
+        //   e = 2 (t k mod n)                   parity 0
+        //   e = 2 (t k mod n) + t               parity 1 forward:  w_n^(t k) w_L^t
+        //   e = 2 (t k mod n) + (k mod A)       parity 1 inverse:  w_n^(t k) w_L^(k mod A)
+        p->tw1_host[a].resize(3 * (size_t)n);
         const long double two_pi = 6.283185307179586476925286766559005768L;
-        for (int k = 0; k < 16; ++k)
-            for (int t = 0; t < A; ++t) {
-                long double th = two_pi * (long double)((t * k) % n) / (long double)n;
-                p->tw1_host[a][k * A + t] = make_double2((double)cosl(th), (double)(-sinl(th)));
-            }
+        for (int region = 0; region < 3; ++region)
+            for (int k = 0; k < 16; ++k)
+                for (int t = 0; t < A; ++t) {
+                    const int e = (2 * ((t * k) % n) + (region == 1 ? t : region == 2 ? k % A : 0)) % L;
+                    long double th = two_pi * (long double)e / (long double)L;
+                    p->tw1_host[a][(size_t)region * n + k * A + t] = make_double2((double)cosl(th), (double)(-sinl(th)));
+                }
     }
     // P1/P5 run along z and need 16 real columns per CTA; P2/P4 along y; P3 along x (nx = 256 only)
     p->fast[0] = p->fast[4] = p->r16A[2] != 0 && nx >= 16;
@@ -246,15 +251,6 @@ static void release_device(dks_poisson_plan *p)
 extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
 {
     if (!p) return;
-    if (p->dbg) {
-        unsigned long long h[6];
-        if (cudaMemcpy(h, p->dbg, sizeof(h), cudaMemcpyDeviceToHost) == cudaSuccess) {
-            double tot = 0; for (int i = 0; i < 6; ++i) tot += (double)h[i];
-            fprintf(stderr, "dks: fused stage clocks S1 %.1f%% bar %.1f%% | S2 %.1f%% bar %.1f%% | S3 %.1f%% bar %.1f%%\n", 100 * h[0] / tot,
-                    100 * h[1] / tot, 100 * h[2] / tot, 100 * h[3] / tot, 100 * h[4] / tot, 100 * h[5] / tot);
-        }
-        cudaFree(p->dbg);
-    }
     release_device(p);
     delete p;
 }
@@ -291,13 +287,6 @@ static int fused_prepare(dks_poisson_plan *p)
     int n = 0;
     DKS_CUDA(cudaOccupancyMaxActiveClusters(&n, p234_fused_r16<A, CL>, &cfg));
     p->fused_clusters = n;
-    if (getenv("DKS_DEBUG")) {
-        fprintf(stderr, "dks: fused A=%d: %d co-resident clusters of %d CTAs\n", A, n, CL);
-        if (getenv("DKS_STAGE_CLOCKS") && !p->dbg) {
-            DKS_CUDA(cudaMalloc(&p->dbg, 6 * sizeof(unsigned long long)));
-            DKS_CUDA(cudaMemset(p->dbg, 0, 6 * sizeof(unsigned long long)));
-        }
-    }
     return DKS_OK;
 }
 
@@ -312,12 +301,12 @@ static int fused_launch(const dks_poisson_plan *p, cudaStream_t st)
     cfg.gridDim = dim3(CL * clusters); cfg.blockDim = dim3(kFusedThreads); cfg.dynamicSmemBytes = kFusedSmem;
     cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
     DKS_CUDA(cudaLaunchKernelEx(&cfg, p234_fused_r16<A, CL>, p->A, p->B, (const double *)p->G, p->d, (const cplx *)p->tw1[0],
-                                (const cplx *)p->tw[0], (const cplx *)p->tw1[1], (const cplx *)p->tw[1], p->dbg, getenv("DKS_FUSED_SKIP") ? atoi(getenv("DKS_FUSED_SKIP")) : 0));
+                                (const cplx *)p->tw1[1]));
     return DKS_OK;
 }
 
 // (A, cluster size) instantiations
-#define DKS_FOR_EACH_FUSED(X) X(4, 4) X(8, 4) X(16, 4) X(4, 8) X(8, 8) X(16, 8) X(16, 2) X(16, 16)
+#define DKS_FOR_EACH_FUSED(X) X(4, 4) X(8, 4) X(16, 4)
 
 template <int A>
 static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
@@ -410,7 +399,6 @@ static int ensure_device(dks_poisson_plan *p)
     int rc = r16_set_attributes();
     if (rc) return rc;
     if (p->fused_ok) {
-        if (const char *e = getenv("DKS_FUSED_CL")) p->fused_cl = atoi(e);
 #define X(A_, CL_) if (p->r16A[1] == A_ && p->fused_cl == CL_) rc = fused_prepare<A_, CL_>(p);
         DKS_FOR_EACH_FUSED(X)
 #undef X
