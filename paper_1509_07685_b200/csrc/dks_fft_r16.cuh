@@ -143,6 +143,31 @@ __device__ __forceinline__ void fft_second(cplx (&v)[16])
     for (int r = 0; r < 16; ++r) v[r] = o[r];
 }
 
+// Transpose of fft_second (the DFT matrix is symmetric, so only the register permutation is mirrored):
+// v[g + (16/A) k_a] -> radix-A over k_a -> v[g A + a'].  First step of the transposed inverse flow.
+template <int A, int SIGN>
+__device__ __forceinline__ void fft_second_t(cplx (&v)[16])
+{
+    if (A == 16) {
+        fft16<SIGN>(v);
+        return;
+    }
+    constexpr int G = 16 / A;
+    cplx o[16];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ka = 0; ka < A; ++ka) o[g * A + ka] = v[g + G * ka];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = o[r];
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        if (A == 8) bfly8<SIGN, 1>(&v[g * 8]);
+        if (A == 4) bfly4<SIGN>(v[g * 4], v[g * 4 + 1], v[g * 4 + 2], v[g * 4 + 3]);
+        if (A == 2) bfly2<SIGN>(v[g * 2], v[g * 2 + 1]);
+    }
+}
+
 // Twiddle between the two steps: v[k] *= T[k A + a] (SIGN < 0) or conj(T[k A + a]) (SIGN > 0), k = 0..15.
 // T is one of the three n-entry regions of the per-axis table tw1 (host: build_tw1 in dks_poisson.cu):
 //   [0, n)    parity 0, both directions:  w_n^(a k)

@@ -238,34 +238,45 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 }
 
 // ---------------------------------------------------------------------------------------------
-// P3 for nx = 256: forward x, multiply by the Green's transform, inverse x, crop; in place on B.
-// Persistent: one CTA of 12 warps per SM; every warp runs its own software pipeline over lines
-// line = warp_global + i * warps_total.  While a warp transforms line i, the bulk-copy engine brings
-// line i+1 (4 KB) and its Ghat row into the warp's shared-memory stage (cp.async.bulk + mbarrier), so
-// no DRAM latency is exposed and no register is spent on prefetching.  lane -> a = lane & 15,
-// p = lane >> 4.  The between-step twiddles depend only on the lane and stay in registers.
-// Exchange buffer per warp: ex[p][k][a ^ (k & 7)] (XOR swizzle: conflict free both ways, no padding).
+// P3 for nx = 16 A: forward x, multiply by the Green's transform, inverse x, crop; in place on B.
+// Persistent: one CTA of 12 warps per SM; every warp runs its own software pipeline over GROUPS of
+// J = 16 / A consecutive lines (256 complex = 4 KB of contiguous memory whatever A is):
+// group = warp_global + i * warps_total.  While a warp transforms group i, the bulk-copy engine brings
+// group i+1 and its J Ghat rows into the warp's shared-memory stage (cp.async.bulk + mbarrier), so no
+// DRAM latency is exposed and no register is spent on prefetching.
+// lane -> a = lane % A, p = (lane / A) % 2, j = lane / (2 A) (line within the group).
+// Twiddles: tb[k] = region p of tw1 (see twiddle_between), fixed per lane, in registers.  The inverse runs
+// the TRANSPOSED flow (radix-A, exchange, conj tb, radix-16), in which the same per-lane set applies, so
+// one register set serves both directions and the parity twiddle w_L^(+-m) needs no table at all.
+// Exchange buffer per warp: region (j, p) = [16][A] elements, column XOR-swizzled with the row and regions
+// padded by A elements for A < 8: conflict free in both directions.
 // ---------------------------------------------------------------------------------------------
 constexpr int kP3Warps = 12;
-constexpr int kP3GhatBytes = 2064;                 // 258 doubles >= nx + 1, multiple of 16
-constexpr int kP3OffEx = 4096;                     // after the 256-element line stage
-constexpr int kP3OffG = kP3OffEx + 8192;
-constexpr int kP3OffBar = kP3OffG + kP3GhatBytes;
-constexpr int kP3SmemPerWarp = kP3OffBar + 16;     // 14368
+constexpr int kP3OffEx = 4096;                     // after the 256-element group stage
+constexpr int kP3ExBytes = 2 * 16 * 17 * 16;       // 2 J regions of 17 A elements = 544 elements
+constexpr int kP3OffG = kP3OffEx + kP3ExBytes;     // 12800
+constexpr int kP3GBytes = 2560;                    // J rows of (16 A + 8) doubles: 2112 (A=16) .. 2560 (A=2)
+constexpr int kP3OffBar = kP3OffG + kP3GBytes;     // 15360
+constexpr int kP3SmemPerWarp = kP3OffBar + 128;    // 15488
 constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp;
 
+template <int A>
 __global__ void __launch_bounds__(kP3Warps * 32, 1)
 p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, int planes,
-              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
+              const cplx *__restrict__ tw1)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int A = 16, N = 256, L = 512;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, a = lane & 15, p = lane >> 4;
+    constexpr int N = 16 * A, L = 32 * A, J = 16 / A, G = 16 / A;
+    constexpr int REG = 16 * A + (A < 8 ? A : 0);      // exchange region stride (elements)
+    constexpr int SWZ = A >= 8 ? 7 : A - 1;
+    constexpr unsigned ROWB = (16 * A + 8) * 8;        // bytes of one Ghat row (gpitch doubles)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int a = lane & (A - 1), p = (lane / A) & 1, j = lane / (2 * A);
     unsigned char *wb = smem_raw + warp * kP3SmemPerWarp;
-    const cplx *stage = reinterpret_cast<const cplx *>(wb);
-    cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + p * 256;
-    const double *gs = reinterpret_cast<const double *>(wb + kP3OffG);
-    uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] line data, [1] Ghat row
+    const cplx *stage = reinterpret_cast<const cplx *>(wb) + j * N;
+    cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * REG;
+    const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * (16 * A + 8);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] group data, [1] Ghat rows
     if (lane == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
@@ -273,74 +284,75 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     }
     __syncthreads();
 
-    const unsigned ny2 = 2 * d.ny, nlines = (unsigned)planes * ny2, stride = gridDim.x * kP3Warps;
-    unsigned line = blockIdx.x * kP3Warps + warp;
-    auto ghat_row = [&](unsigned l) {
-        const int kz = kz0 + (int)(l / ny2), ky = (int)(l % ny2);
-        return Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch;
+    const unsigned ny2 = 2 * d.ny, ngroups = (unsigned)planes * ny2 / J, stride = gridDim.x * kP3Warps;
+    unsigned grp = blockIdx.x * kP3Warps + warp;
+    auto fetch_group = [&](unsigned g) {
+        mbar_expect_tx(&bar[0], 256 * sizeof(cplx));
+        bulk_g2s(wb, B + (size_t)g * 256, 256 * sizeof(cplx), &bar[0]);
     };
-    if (lane == 0 && line < nlines) {
-        mbar_expect_tx(&bar[0], N * sizeof(cplx));
-        bulk_g2s(wb, B + (size_t)line * N, N * sizeof(cplx), &bar[0]);
-        mbar_expect_tx(&bar[1], kP3GhatBytes);
-        bulk_g2s(wb + kP3OffG, ghat_row(line), kP3GhatBytes, &bar[1]);
+    auto fetch_ghat = [&](unsigned g) {
+        const unsigned l0 = g * J;
+        const int kz = kz0 + (int)(l0 / ny2), ky0 = (int)(l0 % ny2);
+        mbar_expect_tx(&bar[1], J * ROWB);
+#pragma unroll
+        for (int jj = 0; jj < J; ++jj) {
+            const int ky = ky0 + jj;
+            bulk_g2s(wb + kP3OffG + jj * ROWB, Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch, ROWB, &bar[1]);
+        }
+    };
+    if (lane == 0 && grp < ngroups) {
+        fetch_group(grp);
+        fetch_ghat(grp);
     }
-    // Between-step twiddles, fixed per lane: tb[k] = w_256^(a k) for parity 0, w_256^(a k) w_512^a for parity 1
-    // (regions 0 and 1 of tw1, see twiddle_between).  The inverse runs the TRANSPOSED flow (radix-16,
-    // exchange, twiddle, radix-16), in which the same per-lane set applies conjugated, so one register
-    // set serves both directions and the parity twiddle w_512^(+-m) needs no table: its lane part is in
-    // tb, its register part w_32^b is a compile-time constant (parity_consts).
     cplx tb[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) tb[k] = __ldg(&tw1[p * N + k * A + a]);
 
     unsigned phase = 0;
-    for (; line < nlines; line += stride, phase ^= 1) {
-        const unsigned next = line + stride;
-        cplx *base = B + (size_t)line * N;
+    for (; grp < ngroups; grp += stride, phase ^= 1) {
+        const unsigned next = grp + stride;
+        cplx *base = B + (size_t)grp * 256 + j * N;
         cplx v[16];
         mbar_wait(&bar[0], phase);
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[a + A * b];
         __syncwarp();                                 // stage consumed (and last exchange reads done)
-        if (lane == 0 && next < nlines) {
-            mbar_expect_tx(&bar[0], N * sizeof(cplx));
-            bulk_g2s(wb, B + (size_t)next * N, N * sizeof(cplx), &bar[0]);
-        }
-        // forward
+        if (lane == 0 && next < ngroups) fetch_group(next);
+        // forward: v[b] = x[a + A b] -> v[r] = X[2 (a + A r) + p]
         if (p) parity_consts<-1>(v);
         fft16<-1>(v);
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = cmul(v[k], tb[k]);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
+        for (int k = 0; k < 16; ++k) ex[k * A + (a ^ (k & SWZ))] = v[k];
         __syncwarp();
 #pragma unroll
-        for (int ap = 0; ap < 16; ++ap) v[ap] = ex[a * 16 + (ap ^ (a & 7))];
-        fft16<-1>(v);
-        // multiply: v[r] = X[K], K = 2 (a + 16 r) + p
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[(a + A * g) * A + (ap ^ (a & SWZ))];
+        fft_second<A, -1>(v);
+        // multiply by the real, even Green's transform
         mbar_wait(&bar[1], phase);
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const int K = 2 * (a + A * r) + p;
             v[r] = cscale(v[r], gs[min(K, L - K)]);
         }
-        __syncwarp();                                 // Ghat row consumed, forward exchange reads done
-        if (lane == 0 && next < nlines) {
-            mbar_expect_tx(&bar[1], kP3GhatBytes);
-            bulk_g2s(wb + kP3OffG, ghat_row(next), kP3GhatBytes, &bar[1]);
-        }
-        // inverse, transposed flow: v[r] = X[2 (a + 16 r) + p] -> radix-16 over r -> exchange -> conj tb -> radix-16
-        fft16<+1>(v);
+        __syncwarp();                                 // Ghat rows consumed, forward exchange reads done
+        if (lane == 0 && next < ngroups) fetch_ghat(next);
+        // inverse, transposed flow: radix-A, exchange back, conj tb, radix-16
+        fft_second_t<A, +1>(v);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) ex[k * 16 + (a ^ (k & 7))] = v[k];
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int ap = 0; ap < A; ++ap) ex[(a + A * g) * A + (ap ^ (a & SWZ))] = v[g * A + ap];
         __syncwarp();
 #pragma unroll
-        for (int ap = 0; ap < 16; ++ap) v[ap] = cmulc(ex[a * 16 + (ap ^ (a & 7))], tb[ap]);
+        for (int k = 0; k < 16; ++k) v[k] = cmulc(ex[k * A + (a ^ (k & SWZ))], tb[k]);
         fft16<+1>(v);
         if (p) parity_consts<+1>(v);
         cplx out[8];
-        combine_parities<16>(v, p, out);
+        combine_parities<A>(v, p, out);
 #pragma unroll
         for (int i = 0; i < 8; ++i) stg_stream(&base[a + A * (i + 8 * p)], out[i]);
     }

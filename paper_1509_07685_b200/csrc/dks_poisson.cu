@@ -211,7 +211,7 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     // P1/P5 run along z and need 16 real columns per CTA; P2/P4 along y; P3 along x (nx = 256 only)
     p->fast[0] = p->fast[4] = p->r16A[2] != 0 && nx >= 16;
     p->fast[1] = p->fast[3] = p->r16A[1] != 0;
-    p->fast[2] = p->r16A[0] == 16;
+    p->fast[2] = p->r16A[0] != 0;
     // tile widths: lines along x are tiled over ky (2ny >= 16 of them per plane); lines along y / z are
     // tiled over x (nx complex columns, or nx/2 packed real pairs for the z passes)
     p->Wx = tile_width_for(2 * nx);
@@ -221,7 +221,7 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
     p->slab = auto_slab(p);
-    p->fused_ok = p->fast[1] && p->fast[2] && p->r16A[1] >= 4;
+    p->fused_ok = p->fast[1] && p->r16A[0] == 16 && p->r16A[1] >= 4;
     p->use_fused = false;               // measured slower than the separate passes so far: opt-in
     compute_layout(p);
     g_err[0] = 0;
@@ -266,10 +266,10 @@ static int r16_set_attributes()
     DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
-    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem));
     DKS_FOR_EACH_A(X)
 #undef X
-    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem));
     return DKS_OK;
 }
 
@@ -331,9 +331,13 @@ static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *
 {
     if (s.pass == 3) {
         const MeshDims d = p->d;
-        const unsigned lines = (unsigned)s.planes * 2 * d.ny;
-        const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (lines + kP3Warps - 1) / kP3Warps);
-        p3_x_conv_r16<<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, s.kz0, s.planes, p->tw1[0], p->tw[0]);
+        const unsigned groups = (unsigned)s.planes * 2 * d.ny / (16 / p->r16A[0]);      // 256 complex each
+        const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (groups + kP3Warps - 1) / kP3Warps);
+        switch (p->r16A[0]) {
+#define X(A_) case A_: p3_x_conv_r16<A_><<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, s.kz0, s.planes, p->tw1[0]); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
         return;
     }
     const int A = (s.pass == 1 || s.pass == 5) ? p->r16A[2] : p->r16A[1];
