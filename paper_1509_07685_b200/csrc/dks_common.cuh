@@ -42,6 +42,17 @@ __device__ __forceinline__ void stg_stream(cplx *p, cplx v)
     asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
 
+// two neighbouring complex values with one 256-bit access (sm_100: LDG.256 / STG.256); p is 32-byte aligned
+__device__ __forceinline__ void stg_stream2(cplx *p, cplx v0, cplx v1)
+{
+    asm volatile("st.global.L1::no_allocate.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v0.x), "d"(v0.y), "d"(v1.x), "d"(v1.y)
+                 : "memory");
+}
+__device__ __forceinline__ void ldg_stream2(const cplx *p, cplx &v0, cplx &v1)
+{
+    asm volatile("ld.global.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v0.x), "=d"(v0.y), "=d"(v1.x), "=d"(v1.y) : "l"(p));
+}
+
 // Ampere-style asynchronous 16-byte copy global -> shared (SASS LDGSTS), bypassing L1 and registers.
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 {

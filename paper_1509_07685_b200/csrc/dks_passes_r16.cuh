@@ -124,7 +124,7 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
 // the packed spectrum C is split with FT{a}[k] = (C[k] + conj C[L-k]) / 2, FT{b}[k] = (C[k] - conj C[L-k]) / (2i).
 // Persistent: CTA t, t + grid, ... over the (nx / 16) * ny tiles of 16 real columns.  The next tile's
 // rho rows (N rows x 128 B) arrive in the shared-memory stage through cp.async while this tile is
-// transformed, so the DRAM latency is never exposed.  Split output: 16 lanes store one 256-byte row.
+// transformed, so the DRAM latency is never exposed.  Split output: one 256-bit store per thread (FT{a}[k], FT{b}[k] are neighbours), 8 lanes = one 256-byte row.
 // ---------------------------------------------------------------------------------------------
 template <int A>
 struct P1Geom {
@@ -180,12 +180,11 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
 #pragma unroll
         for (int r = 0; r < 16; ++r) ex[(2 * (a + A * r) + p) * kCols + c] = v[r];
         __syncthreads();
-        for (int idx = tid; idx < (N + 1) * 2 * kCols; idx += THREADS) {
-            const int k = idx >> 4, j = idx & 15, cc = j >> 1;
+        for (int idx = tid; idx < (N + 1) * kCols; idx += THREADS) {
+            const int k = idx >> 3, cc = idx & 7;
             const cplx ck = ex[k * kCols + cc], cm = ex[((L - k) & (L - 1)) * kCols + cc];
-            const cplx o = (j & 1) ? cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x))
-                                   : cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y));
-            stg_stream(&Aout[((size_t)k * ny + y) * nx + x0 + j], o);
+            stg_stream2(&Aout[((size_t)k * ny + y) * nx + x0 + 2 * cc], cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
+                        cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x)));
         }
     }
 }
