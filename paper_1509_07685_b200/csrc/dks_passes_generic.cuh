@@ -186,6 +186,8 @@ __global__ void greens_fill_kernel(double *__restrict__ G, MeshDims d, double hx
 // One axis of the transform of the even extension (i' = min(i, 2n-i), PAPER.md:98 / reading A4):
 // out[k] = sum_{p<2n} g[min(p, 2n-p)] e^{-2 pi i p k / 2n}, k = 0..n, which is real.  In place.
 // Lines are enumerated as l = b * na + a with base offset a*sa + b*sb; elements at stride es.
+// Two lines share one complex transform: the transform of a real EVEN sequence is real, so for
+// c = g1 + i g2 simply FT{g1} = Re FT{c} and FT{g2} = Im FT{c}; slot w of a CTA carries lines 2(l0+w), +1.
 __global__ void __launch_bounds__(256)
 greens_axis_kernel(double *__restrict__ G, int n, int logL, int W, long long es, int na, long long sa,
                    int nb, long long sb, double scale, const cplx *__restrict__ tw)
@@ -193,20 +195,24 @@ greens_axis_kernel(double *__restrict__ G, int n, int logL, int W, long long es,
     extern __shared__ cplx s[];
     const int L = 2 * n, WP = W + 1;
     const int tid = threadIdx.x, nt = blockDim.x;
-    const long long l0 = (long long)blockIdx.x * W, nlines = (long long)na * nb;
+    const long long l0 = 2 * (long long)blockIdx.x * W, nlines = (long long)na * nb;
     for (int idx = tid; idx < L * W; idx += nt) {
         int p = idx / W, w = idx % W;
-        long long l = l0 + w;
-        double v = 0.0;
-        if (l < nlines) v = G[(l % na) * sa + (l / na) * sb + (long long)min(p, L - p) * es];
-        s[p * WP + w] = cmake(v, 0.0);
+        long long l1 = l0 + 2 * w, l2 = l1 + 1;
+        const long long e = (long long)min(p, L - p) * es;
+        double v1 = 0.0, v2 = 0.0;
+        if (l1 < nlines) v1 = G[(l1 % na) * sa + (l1 / na) * sb + e];
+        if (l2 < nlines) v2 = G[(l2 % na) * sa + (l2 / na) * sb + e];
+        s[p * WP + w] = cmake(v1, v2);
     }
     __syncthreads();
     tile_fft_dif<-1>(s, L, logL, W, WP, tw);
     for (int idx = tid; idx < (n + 1) * W; idx += nt) {
         int k = idx / W, w = idx % W;
-        long long l = l0 + w;
-        if (l < nlines) G[(l % na) * sa + (l / na) * sb + (long long)k * es] = s[brev(k, logL) * WP + w].x * scale;
+        long long l1 = l0 + 2 * w, l2 = l1 + 1;
+        const cplx c = s[brev(k, logL) * WP + w];
+        if (l1 < nlines) G[(l1 % na) * sa + (l1 / na) * sb + (long long)k * es] = c.x * scale;
+        if (l2 < nlines) G[(l2 % na) * sa + (l2 / na) * sb + (long long)k * es] = c.y * scale;
     }
 }
 

@@ -284,12 +284,16 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     __syncthreads();
 
     const unsigned ny2 = 2 * d.ny, ngroups = (unsigned)planes * ny2 / J, stride = gridDim.x * kP3Warps;
+    // Groups are walked from the LAST plane down: P2 has just written B front to back, so its tail is still in
+    // L2 when P3 starts, and P3's own tail (the first planes) is in L2 when P4 starts at plane 0.
     unsigned grp = blockIdx.x * kP3Warps + warp;
-    auto fetch_group = [&](unsigned g) {
+    auto fetch_group = [&](unsigned gi) {
+        const unsigned g = ngroups - 1 - gi;
         mbar_expect_tx(&bar[0], 256 * sizeof(cplx));
         bulk_g2s(wb, B + (size_t)g * 256, 256 * sizeof(cplx), &bar[0]);
     };
-    auto fetch_ghat = [&](unsigned g) {
+    auto fetch_ghat = [&](unsigned gi) {
+        const unsigned g = ngroups - 1 - gi;
         const unsigned l0 = g * J;
         const int kz = kz0 + (int)(l0 / ny2), ky0 = (int)(l0 % ny2);
         mbar_expect_tx(&bar[1], J * ROWB);
@@ -310,7 +314,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     unsigned phase = 0;
     for (; grp < ngroups; grp += stride, phase ^= 1) {
         const unsigned next = grp + stride;
-        cplx *base = B + (size_t)grp * 256 + j * N;
+        cplx *base = B + (size_t)(ngroups - 1 - grp) * 256 + j * N;
         cplx v[16];
         mbar_wait(&bar[0], phase);
 #pragma unroll

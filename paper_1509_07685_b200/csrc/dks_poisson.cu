@@ -533,13 +533,13 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
     {
         long long nl = (long long)(d.ny + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.nx * (W + 1) * sizeof(cplx);
-        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.nx, d.lx, W, 1, d.ny + 1, pitch,
+        greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nx, d.lx, W, 1, d.ny + 1, pitch,
                                                                          d.nz + 1, plane, 1.0, p->tw[0]);
     }
     {
         long long nl = (long long)(d.nx + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.ny * (W + 1) * sizeof(cplx);
-        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.ny, d.ly, W, pitch, d.nx + 1, 1,
+        greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.ny, d.ly, W, pitch, d.nx + 1, 1,
                                                                          d.nz + 1, plane, 1.0, p->tw[1]);
     }
     {
@@ -547,7 +547,7 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
         size_t sm = (size_t)2 * d.nz * (W + 1) * sizeof(cplx);
         // fold hx hy hz / (8 nx ny nz) (Eq. (2)'s prefactor and the inverse transform's 1/N, reading A5)
         const double scale = p->hx * p->hy * p->hz / (8.0 * d.nx * d.ny * d.nz);
-        greens_axis_kernel<<<(unsigned)((nl + W - 1) / W), 256, sm, st>>>(p->G, d.nz, d.lz, W, plane, d.nx + 1, 1,
+        greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nz, d.lz, W, plane, d.nx + 1, 1,
                                                                          d.ny + 1, pitch, scale, p->tw[2]);
     }
     DKS_CUDA(cudaGetLastError());
