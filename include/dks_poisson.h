@@ -77,6 +77,15 @@ int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi
  * The staging buffer is part of the workspace. */
 int dks_poisson_solve_host(dks_poisson_plan *plan, const double *rho_host, double *phi_host, void *stream);
 
+/* The same without the final synchronisation, so that consecutive steps overlap (PAPER.md:132 overlaps the rho
+ * transfer with device work through streams): the copy-in of call i+1 and the copy-out of call i-1 run on
+ * plan-owned streams beside the solve of call i, which runs on `stream`; two staging meshes alternate.  Every
+ * call still moves its own rho and phi.  phi_host of a call is complete after dks_poisson_host_sync (which
+ * waits for every copy-out issued so far); rho_host must stay unchanged until then.  Pinned host memory is
+ * needed for the overlap.  Not capturable in a CUDA graph. */
+int dks_poisson_solve_host_async(dks_poisson_plan *plan, const double *rho_host, double *phi_host, void *stream);
+int dks_poisson_host_sync(dks_poisson_plan *plan);
+
 /* Changes the mesh spacings (they are time dependent).  Invalidates the Green's
  * transform: call dks_greens_setup again before the next solve. */
 int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double hz);
@@ -84,8 +93,8 @@ int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double
 /* Overrides G(0,0,0); NaN restores the default rule.  Invalidates the Green's transform. */
 int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
 
-/* Bytes of device workspace the plan needs (buffer A, the Green's octant, the host-path staging
- * buffer, one slab of B). */
+/* Bytes of device workspace the plan needs (buffer A, the Green's octant, the two host-path staging
+ * meshes, one slab of B). */
 size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
 
 /* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace; 256-byte aligned,

@@ -70,7 +70,11 @@ struct dks_poisson_plan {
     size_t ws_bytes = 0;
     bool ws_owned = false;
     cplx *A = nullptr, *B = nullptr;
-    double *G = nullptr, *stage = nullptr;
+    double *G = nullptr, *stage = nullptr;   // stage: two staging meshes (host path), back to back
+    // host path pipeline (dks_poisson_solve_host_async): copy-in and copy-out streams and per-slot events
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_in[2] = { nullptr, nullptr }, ev_solve[2] = { nullptr, nullptr }, ev_out[2] = { nullptr, nullptr };
+    unsigned long long host_calls = 0;
     size_t offA, offB, offG, offS, need_bytes;
     // P2..P4 run slab by slab (slab = `slab` consecutive kz planes) so that B, the largest intermediate,
     // is a slab-sized scratch that stays resident in L2 between the three passes
@@ -131,7 +135,7 @@ static void compute_layout(dks_poisson_plan *p)
     size_t off = 0;
     p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1), 256);
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
-    p->offS = off; off = align_up(off + 8 * nx * ny * nz, 256);
+    p->offS = off; off = align_up(off + 2 * align_up(8 * nx * ny * nz, 256), 256);
     p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)p->slab, 256);
     p->need_bytes = off;
     p->steps.clear();
@@ -244,6 +248,15 @@ static void release_device(dks_poisson_plan *p)
     p->ws = nullptr; p->ws_owned = false;
     if (p->setup_done) cudaEventDestroy(p->setup_done);
     p->setup_done = nullptr;
+    for (int i = 0; i < 2; ++i) {
+        if (p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
+        if (p->ev_solve[i]) cudaEventDestroy(p->ev_solve[i]);
+        if (p->ev_out[i]) cudaEventDestroy(p->ev_out[i]);
+        p->ev_in[i] = p->ev_solve[i] = p->ev_out[i] = nullptr;
+    }
+    if (p->s_in) cudaStreamDestroy(p->s_in);
+    if (p->s_out) cudaStreamDestroy(p->s_out);
+    p->s_in = p->s_out = nullptr;
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     p->ev.clear();
 }
@@ -691,16 +704,50 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
     return DKS_OK;
 }
 
-extern "C" int dks_poisson_solve_host(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
+// Host path.  Every call copies its rho to the device, solves and copies phi back, but consecutive calls
+// overlap: the copy-in of call i+1 and the copy-out of call i-1 run on their own streams beside the solve
+// of call i (PCIe is full duplex), as PAPER.md:132 does for the rho transfer.  Two staging meshes alternate.
+extern "C" int dks_poisson_solve_host_async(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
 {
     if (!p || !rho_host || !phi_host) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve_host");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!p->s_in) {
+        DKS_CUDA(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking));
+        DKS_CUDA(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            DKS_CUDA(cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming));
+            DKS_CUDA(cudaEventCreateWithFlags(&p->ev_solve[i], cudaEventDisableTiming));
+            DKS_CUDA(cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming));
+        }
+    }
     const size_t bytes = sizeof(double) * (size_t)p->d.nx * p->d.ny * p->d.nz;
-    DKS_CUDA(cudaMemcpyAsync(p->stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
-    int rc = dks_poisson_solve(p, p->stage, p->stage, stream);
+    const int slot = (int)(p->host_calls++ & 1);
+    double *stage = p->stage + (size_t)slot * (align_up(bytes, 256) / sizeof(double));
+    if (p->host_calls > 2) DKS_CUDA(cudaStreamWaitEvent(p->s_in, p->ev_out[slot], 0));   // slot free again
+    DKS_CUDA(cudaMemcpyAsync(stage, rho_host, bytes, cudaMemcpyHostToDevice, p->s_in));
+    DKS_CUDA(cudaEventRecord(p->ev_in[slot], p->s_in));
+    DKS_CUDA(cudaStreamWaitEvent(st, p->ev_in[slot], 0));
+    int rc = dks_poisson_solve(p, stage, stage, stream);
     if (rc) return rc;
-    DKS_CUDA(cudaMemcpyAsync(phi_host, p->stage, bytes, cudaMemcpyDeviceToHost, st));
-    DKS_CUDA(cudaStreamSynchronize(st));
+    DKS_CUDA(cudaEventRecord(p->ev_solve[slot], st));
+    DKS_CUDA(cudaStreamWaitEvent(p->s_out, p->ev_solve[slot], 0));
+    DKS_CUDA(cudaMemcpyAsync(phi_host, stage, bytes, cudaMemcpyDeviceToHost, p->s_out));
+    DKS_CUDA(cudaEventRecord(p->ev_out[slot], p->s_out));
+    // later work on the caller's stream is ordered after this call's copy-out only through dks_poisson_host_sync
     return DKS_OK;
+}
+
+extern "C" int dks_poisson_host_sync(dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (p->s_out) DKS_CUDA(cudaStreamSynchronize(p->s_out));
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_solve_host(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
+{
+    int rc = dks_poisson_solve_host_async(p, rho_host, phi_host, stream);
+    if (rc) return rc;
+    return dks_poisson_host_sync(p);
 }

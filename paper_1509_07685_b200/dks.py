@@ -29,6 +29,8 @@ SYMBOLS = {
     "dks_greens_setup": (_i, [_vp]),
     "dks_poisson_solve": (_i, [_vp, _vp, _vp, _vp]),
     "dks_poisson_solve_host": (_i, [_vp, _vp, _vp, _vp]),
+    "dks_poisson_solve_host_async": (_i, [_vp, _vp, _vp, _vp]),
+    "dks_poisson_host_sync": (_i, [_vp]),
     "dks_poisson_set_spacing": (_i, [_vp, _d, _d, _d]),
     "dks_poisson_set_g0": (_i, [_vp, _d]),
     "dks_poisson_workspace_bytes": (_sz, [_vp]),
@@ -112,6 +114,15 @@ def dks_poisson_solve(plan, rho_dev, phi_dev, stream=None):
 
 def dks_poisson_solve_host(plan, rho_host, phi_host, stream=None):
     return _check(lib.dks_poisson_solve_host(plan, _ptr(rho_host), _ptr(phi_host), stream), "dks_poisson_solve_host")
+
+
+def dks_poisson_solve_host_async(plan, rho_host, phi_host, stream=None):
+    return _check(lib.dks_poisson_solve_host_async(plan, _ptr(rho_host), _ptr(phi_host), stream),
+                  "dks_poisson_solve_host_async")
+
+
+def dks_poisson_host_sync(plan):
+    return _check(lib.dks_poisson_host_sync(plan), "dks_poisson_host_sync")
 
 
 def dks_poisson_set_spacing(plan, hx, hy, hz):
@@ -233,6 +244,16 @@ class PoissonPlan:
 
         dks_poisson_solve_host(self._plan, rho_host, phi_host, torch.cuda.current_stream().cuda_stream)
         return phi_host
+
+    def solve_host_async(self, rho_host, phi_host):
+        """As solve_host without the final wait: consecutive calls overlap their copies; finish with host_sync()."""
+        import torch
+
+        dks_poisson_solve_host_async(self._plan, rho_host, phi_host, torch.cuda.current_stream().cuda_stream)
+        return phi_host
+
+    def host_sync(self):
+        dks_poisson_host_sync(self._plan)
 
     def greens_hat(self):
         import numpy as np

@@ -254,6 +254,24 @@ def test_solve_host_path(torch_cuda, dks, oracle, workloads):
         plan.close()
 
 
+def test_solve_host_async_pipeline(torch_cuda, dks, oracle, workloads):
+    # five pipelined steps with different inputs: every step's phi must be its own (two staging slots alternate)
+    torch = torch_cuda
+    n, h = (32, 16, 64), (2e-4, 3e-4, 1e-4)
+    rhos = [workloads.random_rho(n, seed=40 + i) for i in range(5)]
+    plan = dks.PoissonPlan(n, h)
+    try:
+        h_in = [torch.from_numpy(r).pin_memory() for r in rhos]
+        h_out = [torch.empty_like(t).pin_memory() for t in h_in]
+        for a, b in zip(h_in, h_out):
+            plan.solve_host_async(a, b)
+        plan.host_sync()
+        for r, b in zip(rhos, h_out):
+            check(b.numpy(), oracle.solve(r, n, h, precision="ld"))
+    finally:
+        plan.close()
+
+
 def test_stream_ordering_and_graph_capture(torch_cuda, dks, oracle, workloads):
     torch = torch_cuda
     w = workloads.config(1)
