@@ -177,10 +177,10 @@ __global__ void greens_fill_kernel(double *__restrict__ G, MeshDims d, double hx
                                    double coef, double g0)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i > d.nx) return;
+    if (i >= d.gpitch) return;
     double x = i * hx, y = j * hy, z = k * hz;
     double v = (i == 0 && j == 0 && k == 0) ? g0 : coef / sqrt(x * x + y * y + z * z);
-    G[((size_t)k * (d.ny + 1) + j) * d.gpitch + i] = v;
+    G[((size_t)k * (d.ny + 1) + j) * d.gpitch + i] = i <= d.nx ? v : 0.0;      // pad entries stay zero (dks_greens_r16.cuh)
 }
 
 // One axis of the transform of the even extension (i' = min(i, 2n-i), PAPER.md:98 / reading A4):

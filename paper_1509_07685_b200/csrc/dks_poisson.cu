@@ -20,6 +20,7 @@
 #include "dks_passes_generic.cuh"
 #include "dks_passes_r16.cuh"
 #include "dks_fused_r16.cuh"
+#include "dks_greens_r16.cuh"
 
 using namespace dks;
 
@@ -280,7 +281,9 @@ static int r16_set_attributes()
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
-    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem));
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem)); \
+    DKS_CUDA(cudaFuncSetAttribute(greens_x_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGxSmem)); \
+    DKS_CUDA(cudaFuncSetAttribute(greens_axis_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
     DKS_FOR_EACH_A(X)
 #undef X
     return DKS_OK;
@@ -536,32 +539,52 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
     const double coef = (double)(1.0L / (4.0L * pi_l * 8.8541878128e-12L));
     const double hmin = std::min(p->hx, std::min(p->hy, p->hz));
     const double g0 = std::isnan(p->g0_override) ? coef / (0.5 * hmin) : p->g0_override;
-    {
-        dim3 blk(128), grd((d.nx + 1 + 127) / 128, d.ny + 1, d.nz + 1);
-        greens_fill_kernel<<<grd, blk, 0, st>>>(p->G, d, p->hx, p->hy, p->hz, coef, g0);
-    }
     const long long pitch = d.gpitch, plane = pitch * (d.ny + 1);
     const int W = 4;
-    // x lines: (ky, kz) ; y lines: (kx, kz) ; z lines: (kx, ky)
-    {
+    // fold hx hy hz / (8 nx ny nz) (Eq. (2)'s prefactor and the inverse transform's 1/N, reading A5) into the last axis
+    const double scale = p->hx * p->hy * p->hz / (8.0 * d.nx * d.ny * d.nz);
+    // x lines: (ky, kz) ; y lines: (kx, kz) ; z lines: (kx, ky).  Every axis with n = 32..256 takes the
+    // register-resident kernels of dks_greens_r16.cuh (x: fused with the evaluation of G), the others the generic ones.
+    if (p->r16A[0]) {
+        const unsigned pairs = (unsigned)(d.nz + 1) * ((d.ny + 2) / 2), groups = (pairs + 16 / p->r16A[0] - 1) / (16 / p->r16A[0]);
+        const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (groups + kGxWarps - 1) / kGxWarps);
+        switch (p->r16A[0]) {
+#define X(A_) case A_: greens_x_r16<A_><<<grid, kGxWarps * 32, kGxSmem, st>>>(p->G, d, p->hx, p->hy, p->hz, coef, g0, p->tw1[0]); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+    } else {
+        dim3 blk(128), grd((d.gpitch + 127) / 128, d.ny + 1, d.nz + 1);
+        greens_fill_kernel<<<grd, blk, 0, st>>>(p->G, d, p->hx, p->hy, p->hz, coef, g0);
         long long nl = (long long)(d.ny + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.nx * (W + 1) * sizeof(cplx);
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nx, d.lx, W, 1, d.ny + 1, pitch,
-                                                                         d.nz + 1, plane, 1.0, p->tw[0]);
+                                                                                   d.nz + 1, plane, 1.0, p->tw[0]);
     }
-    {
+    const dim3 xt((d.gpitch + 2 * kCols - 1) / (2 * kCols));
+    if (p->r16A[1]) {
+        switch (p->r16A[1]) {
+#define X(A_) case A_: greens_axis_r16<A_><<<dim3(xt.x, d.nz + 1), R16Geom<A_>::THREADS, R16Geom<A_>::SMEM, st>>>(p->G, d.gpitch, pitch, plane, 1.0, p->tw1[1]); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+    } else {
         long long nl = (long long)(d.nx + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.ny * (W + 1) * sizeof(cplx);
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.ny, d.ly, W, pitch, d.nx + 1, 1,
-                                                                         d.nz + 1, plane, 1.0, p->tw[1]);
+                                                                                   d.nz + 1, plane, 1.0, p->tw[1]);
     }
-    {
+    if (p->r16A[2]) {
+        switch (p->r16A[2]) {
+#define X(A_) case A_: greens_axis_r16<A_><<<dim3(xt.x, d.ny + 1), R16Geom<A_>::THREADS, R16Geom<A_>::SMEM, st>>>(p->G, d.gpitch, plane, pitch, scale, p->tw1[2]); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+    } else {
         long long nl = (long long)(d.nx + 1) * (d.ny + 1);
         size_t sm = (size_t)2 * d.nz * (W + 1) * sizeof(cplx);
-        // fold hx hy hz / (8 nx ny nz) (Eq. (2)'s prefactor and the inverse transform's 1/N, reading A5)
-        const double scale = p->hx * p->hy * p->hz / (8.0 * d.nx * d.ny * d.nz);
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nz, d.lz, W, plane, d.nx + 1, 1,
-                                                                         d.ny + 1, pitch, scale, p->tw[2]);
+                                                                                   d.ny + 1, pitch, scale, p->tw[2]);
     }
     DKS_CUDA(cudaGetLastError());
     DKS_CUDA(cudaEventRecord(p->setup_done, st));
