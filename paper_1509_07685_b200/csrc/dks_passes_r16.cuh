@@ -211,8 +211,7 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
         const int idx = tid + i * THREADS, k = idx >> 3, cc = idx & 7;
         if (idx < ITEMS) {
             const cplx *in = &Ain[((size_t)k * ny + y) * nx + x0 + 2 * cc];
-            fa[i] = ldg_stream(in);
-            fb[i] = ldg_stream(in + 1);
+            ldg_stream2(in, fa[i], fb[i]);            // one 256-bit load: FT{a}[k], FT{b}[k] are neighbours
         }
     }
 #pragma unroll
