@@ -90,23 +90,65 @@ __device__ __forceinline__ void bfly8(cplx *v)
     for (int k = 0; k < 8; ++k) v[k * S] = o[k];
 }
 
-// 16-point DFT in registers, natural order in and out (4 x 4 decomposition, 160 fp64 instructions)
+// x * (1 + S i) and x * (-1 + S i) without the 1/sqrt(2): the 8th roots w16^2 = c (1 + S i), w16^6 = c (-1 + S i),
+// c = 1/sqrt(2), S = SIGN; the factor c is folded into the FMAs of the butterfly that consumes the product.
+template <int SIGN>
+__device__ __forceinline__ cplx rot_p(cplx a) { return SIGN < 0 ? cmake(a.x + a.y, a.y - a.x) : cmake(a.x - a.y, a.y + a.x); }
+template <int SIGN>
+__device__ __forceinline__ cplx rot_m(cplx a) { return SIGN < 0 ? cmake(a.y - a.x, -a.y - a.x) : cmake(-a.x - a.y, a.x - a.y); }
+__device__ __forceinline__ cplx cfma(double s, cplx t, cplx u) { return cmake(fma(s, t.x, u.x), fma(s, t.y, u.y)); }
+
+// 4-point DFT as bfly4, with x2 given as c * t2 (t2 unscaled): the scale rides on the FMAs
+template <int SIGN>
+__device__ __forceinline__ void bfly4_x2scaled(cplx &x0, cplx &x1, cplx &x2, cplx &x3, cplx t2)
+{
+    constexpr double c = 0.70710678118654752440;
+    cplx apc = cfma(c, t2, x0), amc = cfma(-c, t2, x0), bpd = cadd(x1, x3), bmd = mul_si<SIGN>(csub(x1, x3));
+    x0 = cadd(apc, bpd);
+    x1 = cadd(amc, bmd);
+    x2 = csub(apc, bpd);
+    x3 = csub(amc, bmd);
+}
+
+// 16-point DFT in registers, natural order in and out (4 x 4 decomposition, 152 fp64 instructions: the four
+// 8th-root twiddles of the middle layer cost two additions each, their 1/sqrt(2) is folded into FMAs)
+template <int SIGN>
+__device__ __forceinline__ void fft16_tail(cplx (&v)[16]);
+
 template <int SIGN>
 __device__ __forceinline__ void fft16(cplx (&v)[16])
 {
 #pragma unroll
     for (int n0 = 0; n0 < 4; ++n0) bfly4<SIGN>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12]);   // slot n0 + 4 k0
+    fft16_tail<SIGN>(v);
+}
+
+// everything after the first layer of 4-point transforms
+template <int SIGN>
+__device__ __forceinline__ void fft16_tail(cplx (&v)[16])
+{
+    constexpr double c = 0.70710678118654752440;
+    // k0 = 0: no twiddles
+    bfly4<SIGN>(v[0], v[1], v[2], v[3]);
+    // k0 = 1: twiddles w^1, w^2, w^3 on slots 5, 6, 7
     v[5] = mul_w16<SIGN, 1>(v[5]);
-    v[9] = mul_w16<SIGN, 2>(v[9]);
-    v[13] = mul_w16<SIGN, 3>(v[13]);
-    v[6] = mul_w16<SIGN, 2>(v[6]);
-    v[10] = mul_w16<SIGN, 4>(v[10]);
-    v[14] = mul_w16<SIGN, 6>(v[14]);
     v[7] = mul_w16<SIGN, 3>(v[7]);
-    v[11] = mul_w16<SIGN, 6>(v[11]);
+    bfly4_x2scaled<SIGN>(v[4], v[5], v[6], v[7], rot_p<SIGN>(v[6]));
+    // k0 = 2: twiddles w^2, w^4, w^6 on slots 9, 10, 11
+    {
+        const cplx x2 = mul_si<SIGN>(v[10]);                       // w^4 = S i
+        const cplx t1 = rot_p<SIGN>(v[9]), t3 = rot_m<SIGN>(v[11]);
+        const cplx apc = cadd(v[8], x2), amc = csub(v[8], x2);
+        const cplx P = cadd(t1, t3), M = mul_si<SIGN>(csub(t1, t3));
+        v[8] = cfma(c, P, apc);
+        v[9] = cfma(c, M, amc);
+        v[10] = cfma(-c, P, apc);
+        v[11] = cfma(-c, M, amc);
+    }
+    // k0 = 3: twiddles w^3, w^6, w^9 on slots 13, 14, 15
+    v[13] = mul_w16<SIGN, 3>(v[13]);
     v[15] = mul_w16<SIGN, 9>(v[15]);
-#pragma unroll
-    for (int k0 = 0; k0 < 4; ++k0) bfly4<SIGN>(v[4 * k0], v[4 * k0 + 1], v[4 * k0 + 2], v[4 * k0 + 3]);
+    bfly4_x2scaled<SIGN>(v[12], v[13], v[14], v[15], rot_m<SIGN>(v[14]));
     // slot 4 k0 + k1 holds X[k0 + 4 k1]: transpose the 4 x 4 register tile
 #pragma unroll
     for (int i = 0; i < 4; ++i)
