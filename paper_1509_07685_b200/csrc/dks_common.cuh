@@ -53,6 +53,13 @@ __device__ __forceinline__ void ldg_stream2(const cplx *p, cplx &v0, cplx &v1)
     asm volatile("ld.global.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v0.x), "=d"(v0.y), "=d"(v1.x), "=d"(v1.y) : "l"(p));
 }
 
+// Programmatic dependent launch (sm_90+).  Every pass kernel of the solve starts with pdl_trigger(): once all
+// CTAs of a grid have started, the next kernel in the stream may be scheduled into the SMs its tail frees
+// and run its prologue; pdl_wait() then blocks until the previous grid has completed and its memory is
+// visible.  Nothing the previous kernel wrote is read, and nothing it read is overwritten, before pdl_wait().
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // Ampere-style asynchronous 16-byte copy global -> shared (SASS LDGSTS), bypassing L1 and registers.
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
 {

@@ -77,7 +77,7 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
 // ---------------------------------------------------------------------------------------------
 // P2: forward y.  grid (nx / 8, nz + 1), 16 A threads.
 // ---------------------------------------------------------------------------------------------
-template <int A>
+template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int kz0,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
@@ -86,6 +86,10 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;          // kz: plane within the slab
     const size_t x = (size_t)blockIdx.x * kCols + c;
+    if (PDL) {
+        pdl_trigger();
+        pdl_wait();
+    }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
@@ -98,7 +102,7 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
 // ---------------------------------------------------------------------------------------------
 // P4: inverse y, crop to ny.  grid (nx / 8, nz + 1)
 // ---------------------------------------------------------------------------------------------
-template <int A>
+template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, int kz0,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
@@ -107,6 +111,10 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
     const size_t x = (size_t)blockIdx.x * kCols + c;
+    if (PDL) {
+        pdl_trigger();
+        pdl_wait();
+    }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b)
@@ -132,7 +140,7 @@ struct P1Geom {
     static constexpr int SMEM = R16Geom<A>::SMEM + STAGE;
 };
 
-template <int A>
+template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
@@ -153,6 +161,10 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
         cp_async_commit();
     };
     int t = blockIdx.x;
+    if (PDL) {
+        pdl_trigger();
+        pdl_wait();                                       // A is still being read by the previous solve's P5
+    }
     if (t < tiles) prefetch(t);
     for (; t < tiles; t += gridDim.x) {
         const int y = t / xtiles;
@@ -193,7 +205,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
 // P5: inverse z, complex -> real, crop to nz.  Rebuilds the packed spectrum C[k] = Fa[k] + i Fb[k],
 // C[L-k] = conj Fa[k] + i conj Fb[k] in shared memory first.  grid (nx / 16, ny)
 // ---------------------------------------------------------------------------------------------
-template <int A>
+template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
@@ -205,6 +217,10 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
     const size_t x0 = (size_t)blockIdx.x * 2 * kCols;
     // all loads of the tile in flight at once (the last round is ragged: row k = N only)
     constexpr int ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
+    if (PDL) {
+        pdl_trigger();
+        pdl_wait();
+    }
     cplx fa[ROUNDS], fb[ROUNDS];
 #pragma unroll
     for (int i = 0; i < ROUNDS; ++i) {
@@ -258,7 +274,7 @@ constexpr int kP3OffBar = kP3OffG + kP3GBytes;     // 15360
 constexpr int kP3SmemPerWarp = kP3OffBar + 128;    // 15488
 constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp;
 
-template <int A>
+template <int A, bool PDL>
 __global__ void __launch_bounds__(kP3Warps * 32, 1)
 p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, int planes,
               const cplx *__restrict__ tw1)
@@ -275,6 +291,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * REG;
     const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * (16 * A + 8);
     uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] group data, [1] Ghat rows
+    if (PDL) pdl_trigger();
     if (lane == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
@@ -302,6 +319,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             bulk_g2s(wb + kP3OffG + jj * ROWB, Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch, ROWB, &bar[1]);
         }
     };
+    if (PDL) pdl_wait();
     if (lane == 0 && grp < ngroups) {
         fetch_group(grp);
         fetch_ghat(grp);

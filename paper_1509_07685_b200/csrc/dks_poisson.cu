@@ -84,6 +84,7 @@ struct dks_poisson_plan {
     struct Step { int pass, kz0, planes; };     // pass 1..5, or kPassFused = P2+P3+P4 of all planes in one kernel
     // fused P2+P3+P4 (dks_fused_r16.cuh): available for nx = 256 and ny = 64, 128, 256
     bool fused_ok = false, use_fused = false;
+    bool pdl = false;                   // programmatic dependent launch between the r16 passes (small meshes)
     int fused_cl = 4;                   // CTAs per cluster
     int fused_clusters = 0;             // clusters of kFusedCluster CTAs that are co-resident on this device
     std::vector<Step> steps;            // the launch list of one solve
@@ -226,6 +227,7 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
     p->slab = auto_slab(p);
+    p->pdl = (size_t)nx * ny * nz <= ((size_t)1 << 21);
     p->fused_ok = p->fast[1] && p->r16A[0] == 16 && p->r16A[1] >= 4;
     p->use_fused = false;               // measured slower than the separate passes so far: opt-in
     compute_layout(p);
@@ -277,11 +279,16 @@ extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
 static int r16_set_attributes()
 {
 #define X(A_)                                                                                                         \
-    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
-    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
-    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
-    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
-    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem)); \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem)); \
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kP3Smem)); \
     DKS_CUDA(cudaFuncSetAttribute(greens_x_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGxSmem)); \
     DKS_CUDA(cudaFuncSetAttribute(greens_axis_r16<A_>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM));
     DKS_FOR_EACH_A(X)
@@ -324,6 +331,27 @@ static int fused_launch(const dks_poisson_plan *p, cudaStream_t st)
 // (A, cluster size) instantiations
 #define DKS_FOR_EACH_FUSED(X) X(4, 4) X(8, 4) X(16, 4)
 
+// Launch with programmatic stream serialization (programmatic dependent launch): the kernel may be scheduled
+// while the previous kernel in the stream drains; it orders itself with pdl_wait() (dks_common.cuh).
+// Measured: it hides 2-3 us per kernel boundary on the small meshes (128^3: 0.113 -> 0.104 ms, 64^3: 0.037 -> 0.034 ms)
+// but costs 5 % at 256^3, so the plan enables it for meshes of at most 128^3 nodes (`pdl`).
+template <typename... KArgs, typename... Args>
+static void launch_pdl(bool pdl, void (*kernel)(KArgs...), void (*kernel_pdl)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                       cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    if (!pdl) {
+        kernel<<<grid, block, smem, st>>>(static_cast<KArgs>(args)...);
+        return;
+    }
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    (void)cudaLaunchKernelEx(&cfg, kernel_pdl, static_cast<KArgs>(args)...);      // errors surface through cudaGetLastError in the solve
+}
+
 template <int A>
 static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
                                cudaStream_t st)
@@ -333,12 +361,12 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
     switch (s.pass) {
     case 1: {
         const int tiles = d.nx / (2 * kCols) * d.ny, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
-        p1_z_r2c_r16<A><<<std::min(tiles, p->sm_count * per_sm), T, P1Geom<A>::SMEM, st>>>(rho, p->A, d, p->tw1[2], p->tw[2]);
+        launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, p->tw1[2], p->tw[2]);
         break;
     }
-    case 2: p2_y_fwd_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
-    case 4: p4_y_inv_r16<A><<<dim3(d.nx / kCols, s.planes), T, S, st>>>(p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
-    case 5: p5_z_c2r_r16<A><<<dim3(d.nx / (2 * kCols), d.ny), T, S, st>>>(p->A, phi, d, p->tw1[2], p->tw[2]); break;
+    case 2: launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 5: launch_pdl(p->pdl, p5_z_c2r_r16<A, false>, p5_z_c2r_r16<A, true>, dim3(d.nx / (2 * kCols), d.ny), dim3(T), S, st, p->A, phi, d, p->tw1[2], p->tw[2]); break;
     }
 }
 
@@ -350,7 +378,7 @@ static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *
         const unsigned groups = (unsigned)s.planes * 2 * d.ny / (16 / p->r16A[0]);      // 256 complex each
         const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (groups + kP3Warps - 1) / kP3Warps);
         switch (p->r16A[0]) {
-#define X(A_) case A_: p3_x_conv_r16<A_><<<grid, kP3Warps * 32, kP3Smem, st>>>(p->B, p->G, d, s.kz0, s.planes, p->tw1[0]); break;
+#define X(A_) case A_: launch_pdl(p->pdl, p3_x_conv_r16<A_, false>, p3_x_conv_r16<A_, true>, dim3(grid), dim3(kP3Warps * 32), kP3Smem, st, p->B, p->G, d, s.kz0, s.planes, p->tw1[0]); break;
             DKS_FOR_EACH_A(X)
 #undef X
         }
