@@ -122,6 +122,30 @@ def test_shapes_signed_random(torch_cuda, dks, oracle, workloads, n, h):
     check(got, ref)
 
 
+# ---- the paper's own mesh shapes (Table 1: 64x64x32 ... 512x512x256), synthetic Gaussian bunch ----
+@pytest.mark.parametrize("n", [(64, 64, 32), (128, 128, 64), (256, 256, 128)])
+def test_paper_table1_shapes(torch_cuda, dks, oracle, workloads, n):
+    h = (2e-4, 2e-4, 4e-4)
+    rho = workloads.random_rho(n, seed=n[0], signed=False)
+    ref = oracle.solve(rho, n, h, precision="d")           # double build: error ~1e-15, far below the tolerance
+    got = gpu_solve(torch_cuda, dks, rho, n, h)
+    check(got, ref)
+
+
+def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
+    # 512x512x256 (padded 1024x1024x512): x and y run the generic passes (n = 512), z the register-resident ones.
+    # Checked against direct summation of Eq. (2) at sampled nodes (one pass over rho per node).
+    n, h = (512, 512, 256), (1e-4, 1e-4, 2e-4)
+    rho = workloads.random_rho(n, seed=99, signed=False)
+    got = gpu_solve(torch_cuda, dks, rho, n, h)
+    assert np.all(np.isfinite(got))
+    nodes = workloads.sample_nodes(n, 7, count=7)
+    direct = oracle.direct_sum_nodes(rho, n, h, nodes)
+    g = got[nodes[:, 2], nodes[:, 1], nodes[:, 0]]
+    assert np.max(np.abs(g - direct)) <= MAX_ABS_TOL * np.max(np.abs(got))
+    assert np.max(np.abs(g - direct) / np.abs(direct)) <= 1e-11
+
+
 # ---- opt-in variants: fused P2+P3+P4 cluster kernel (nx = 256, ny = 64..256) and slab-by-slab launches ----
 @pytest.mark.parametrize("n,h", [((256, 64, 8), (1e-4, 2e-4, 1e-3)), ((256, 128, 16), (1e-4, 1e-4, 4e-4)),
                                  ((256, 256, 40), (1e-4, 1e-4, 2e-4))])
