@@ -71,6 +71,16 @@ int dks_greens_setup(dks_poisson_plan *plan);
  * slab of kz planes (dks_poisson_set_slab_planes), then P5: 2 + 3 * ceil((nz+1)/slab) kernels. */
 int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, void *stream);
 
+/* Several independent meshes of the same shape and spacing in one call (e.g. neighbouring bunches, PAPER.md:140
+ * ref. [27]): rho_dev and phi_dev hold nbatch meshes back to back ([nbatch][nz][ny][nx]).
+ * Every pass processes the whole batch in one launch (still five launches), so small meshes are no longer
+ * launch-latency bound and all meshes share one Green's transform.  nbatch <= dks_poisson_set_max_batch, which
+ * sizes the workspace (A and B scale with it; default 1) and must be called before the workspace is attached /
+ * before dks_greens_setup.  Needs the default pipeline (no slabs, no fused kernel).  Same stream semantics as
+ * dks_poisson_solve; phi_dev may alias rho_dev. */
+int dks_poisson_set_max_batch(dks_poisson_plan *plan, int nbatch);
+int dks_poisson_solve_batch(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, int nbatch, void *stream);
+
 /* Same solve with HOST buffers (the end-to-end path of the paper: rho is copied to
  * the device and phi back every step).  rho_host/phi_host: host pointers ([nz][ny][nx] fp64; pinned
  * memory recommended).  Copies H2D, solves, copies D2H on `stream`, then synchronises the stream.

@@ -33,6 +33,8 @@ p1_z_r2c_generic(const double *__restrict__ rho, cplx *__restrict__ A, MeshDims 
     const int nx = d.nx, ny = d.ny, nz = d.nz, L = 2 * nz, logL = d.lz;
     const int x0 = blockIdx.x * 2 * W, y = blockIdx.y;
     const int tid = threadIdx.x, nt = blockDim.x;
+    rho += (size_t)blockIdx.z * nz * ny * nx;             // blockIdx.z: mesh of the batch
+    A += (size_t)blockIdx.z * (nz + 1) * ny * nx;
     for (int idx = tid; idx < nz * W; idx += nt) {
         int r = idx / W, w = idx % W;
         s[r * W + w] = *reinterpret_cast<const cplx *>(&rho[((size_t)r * ny + y) * nx + x0 + 2 * w]);
@@ -66,6 +68,8 @@ p5_z_c2r_generic(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims 
     const int nx = d.nx, ny = d.ny, nz = d.nz, L = 2 * nz, logL = d.lz;
     const int x0 = blockIdx.x * 2 * W, y = blockIdx.y;
     const int tid = threadIdx.x, nt = blockDim.x;
+    A += (size_t)blockIdx.z * (nz + 1) * ny * nx;         // blockIdx.z: mesh of the batch
+    phi += (size_t)blockIdx.z * nz * ny * nx;
     for (int idx = tid; idx < (nz + 1) * W; idx += nt) {
         int k = idx / W, w = idx % W;
         const cplx *in = &A[((size_t)k * ny + y) * nx + x0 + 2 * w];
@@ -142,7 +146,7 @@ p3_x_conv_generic(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDim
     extern __shared__ cplx s[];
     const int nx = d.nx, ny = d.ny, L = 2 * nx, logL = d.lx, WP = W + 1;
     const int line0 = blockIdx.x * W;
-    const int kz = kz0 + line0 / (2 * ny), ky0 = line0 % (2 * ny);    // line0 counts within the slab
+    const int kz = (kz0 + line0 / (2 * ny)) % (d.nz + 1), ky0 = line0 % (2 * ny);    // line0 counts within the slab; a batch repeats kz
     const int tid = threadIdx.x, nt = blockDim.x;
     cplx *base = B + (size_t)line0 * nx;
     for (int idx = tid; idx < nx * W; idx += nt) {

@@ -142,21 +142,22 @@ struct P1Geom {
 
 template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
-p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d,
+p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d, int nb,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     extern __shared__ cplx ex[];
     constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
     cplx *stage = ex + L * kCols;
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
-    const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny;
+    const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny * nb;   // nb meshes back to back
     auto prefetch = [&](int t) {
-        const int y = t / xtiles;
+        const int yy = t / xtiles, y = yy % ny;
+        const double *src = rho + (size_t)(yy / ny) * N * ny * nx;
         const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
 #pragma unroll
         for (int i = 0; i < N * kCols / THREADS; ++i) {
             const int idx = tid + i * THREADS, r = idx >> 3, cc = idx & 7;
-            cp_async16(&stage[idx], &rho[((size_t)r * ny + y) * nx + x0 + 2 * cc]);
+            cp_async16(&stage[idx], &src[((size_t)r * ny + y) * nx + x0 + 2 * cc]);
         }
         cp_async_commit();
     };
@@ -167,7 +168,8 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aout, MeshDims d
     }
     if (t < tiles) prefetch(t);
     for (; t < tiles; t += gridDim.x) {
-        const int y = t / xtiles;
+        const int yy = t / xtiles, y = yy % ny;
+        cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx;
         const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
         cp_async_wait_all();
         __syncthreads();                                  // stage complete; last tile's split reads done
@@ -215,6 +217,8 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
     const int nx = d.nx, ny = d.ny, y = blockIdx.y;
     const size_t x0 = (size_t)blockIdx.x * 2 * kCols;
+    Ain += (size_t)blockIdx.z * (N + 1) * ny * nx;        // blockIdx.z: mesh of the batch
+    phi += (size_t)blockIdx.z * N * ny * nx;
     // all loads of the tile in flight at once (the last round is ragged: row k = N only)
     constexpr int ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
     if (PDL) {
@@ -311,7 +315,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     auto fetch_ghat = [&](unsigned gi) {
         const unsigned g = ngroups - 1 - gi;
         const unsigned l0 = g * J;
-        const int kz = kz0 + (int)(l0 / ny2), ky0 = (int)(l0 % ny2);
+        const int kz = (kz0 + (int)(l0 / ny2)) % (d.nz + 1), ky0 = (int)(l0 % ny2);   // planes of a batch repeat kz
         mbar_expect_tx(&bar[1], J * ROWB);
 #pragma unroll
         for (int jj = 0; jj < J; ++jj) {

@@ -84,6 +84,7 @@ struct dks_poisson_plan {
     struct Step { int pass, kz0, planes; };     // pass 1..5, or kPassFused = P2+P3+P4 of all planes in one kernel
     // fused P2+P3+P4 (dks_fused_r16.cuh): available for nx = 256 and ny = 64, 128, 256
     bool fused_ok = false, use_fused = false;
+    int max_batch = 1;                  // meshes per dks_poisson_solve_batch call the workspace is sized for
     bool pdl = false;                   // programmatic dependent launch between the r16 passes (small meshes)
     int fused_cl = 4;                   // CTAs per cluster
     int fused_clusters = 0;             // clusters of kFusedCluster CTAs that are co-resident on this device
@@ -135,10 +136,11 @@ static void compute_layout(dks_poisson_plan *p)
 {
     const size_t nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
     size_t off = 0;
-    p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1), 256);
+    const size_t nbm = (size_t)p->max_batch;
+    p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1) * nbm, 256);
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
     p->offS = off; off = align_up(off + 2 * align_up(8 * nx * ny * nz, 256), 256);
-    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)p->slab, 256);
+    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)p->slab * nbm, 256);
     p->need_bytes = off;
     p->steps.clear();
     p->steps.push_back({ 1, 0, 0 });
@@ -354,31 +356,31 @@ static void launch_pdl(bool pdl, void (*kernel)(KArgs...), void (*kernel_pdl)(KA
 
 template <int A>
 static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
-                               cudaStream_t st)
+                               int nb, cudaStream_t st)
 {
     const MeshDims d = p->d;
     const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
     switch (s.pass) {
     case 1: {
-        const int tiles = d.nx / (2 * kCols) * d.ny, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
-        launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, p->tw1[2], p->tw[2]);
+        const int tiles = d.nx / (2 * kCols) * d.ny * nb, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
+        launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, nb, p->tw1[2], p->tw[2]);
         break;
     }
-    case 2: launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
-    case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
-    case 5: launch_pdl(p->pdl, p5_z_c2r_r16<A, false>, p5_z_c2r_r16<A, true>, dim3(d.nx / (2 * kCols), d.ny), dim3(T), S, st, p->A, phi, d, p->tw1[2], p->tw[2]); break;
+    case 2: launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 5: launch_pdl(p->pdl, p5_z_c2r_r16<A, false>, p5_z_c2r_r16<A, true>, dim3(d.nx / (2 * kCols), d.ny, nb), dim3(T), S, st, p->A, phi, d, p->tw1[2], p->tw[2]); break;
     }
 }
 
 static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
-                       cudaStream_t st)
+                       int nb, cudaStream_t st)
 {
     if (s.pass == 3) {
         const MeshDims d = p->d;
-        const unsigned groups = (unsigned)s.planes * 2 * d.ny / (16 / p->r16A[0]);      // 256 complex each
+        const unsigned groups = (unsigned)s.planes * nb * 2 * d.ny / (16 / p->r16A[0]);      // 256 complex each
         const unsigned grid = std::min<unsigned>((unsigned)p->sm_count, (groups + kP3Warps - 1) / kP3Warps);
         switch (p->r16A[0]) {
-#define X(A_) case A_: launch_pdl(p->pdl, p3_x_conv_r16<A_, false>, p3_x_conv_r16<A_, true>, dim3(grid), dim3(kP3Warps * 32), kP3Smem, st, p->B, p->G, d, s.kz0, s.planes, p->tw1[0]); break;
+#define X(A_) case A_: launch_pdl(p->pdl, p3_x_conv_r16<A_, false>, p3_x_conv_r16<A_, true>, dim3(grid), dim3(kP3Warps * 32), kP3Smem, st, p->B, p->G, d, s.kz0, s.planes * nb, p->tw1[0]); break;
             DKS_FOR_EACH_A(X)
 #undef X
         }
@@ -386,23 +388,23 @@ static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *
     }
     const int A = (s.pass == 1 || s.pass == 5) ? p->r16A[2] : p->r16A[1];
     switch (A) {
-#define X(A_) case A_: launch_strided_r16<A_>(s, p, rho, phi, st); break;
+#define X(A_) case A_: launch_strided_r16<A_>(s, p, rho, phi, nb, st); break;
         DKS_FOR_EACH_A(X)
 #undef X
     }
 }
 
 static void launch_generic(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
-                           cudaStream_t st)
+                           int nb, cudaStream_t st)
 {
     const MeshDims d = p->d;
     switch (s.pass) {
-    case 1: p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]); break;
-    case 2: p2_y_fwd_generic<<<dim3(d.nx / p->Wy, s.planes), 256, p->smem_y, st>>>(p->A, p->B, d, s.kz0, p->Wy, p->tw[1]); break;
-    case 3: p3_x_conv_generic<<<(unsigned)((size_t)s.planes * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, s.kz0,
+    case 1: p1_z_r2c_generic<<<dim3(d.nx / (2 * p->Wz), d.ny, nb), 256, p->smem_z, st>>>(rho, p->A, d, p->Wz, p->tw[2]); break;
+    case 2: p2_y_fwd_generic<<<dim3(d.nx / p->Wy, s.planes * nb), 256, p->smem_y, st>>>(p->A, p->B, d, s.kz0, p->Wy, p->tw[1]); break;
+    case 3: p3_x_conv_generic<<<(unsigned)((size_t)s.planes * nb * 2 * d.ny / p->Wx), 256, p->smem_x, st>>>(p->B, p->G, d, s.kz0,
                                                                                                     p->Wx, p->tw[0]); break;
-    case 4: p4_y_inv_generic<<<dim3(d.nx / p->Wy, s.planes), 256, p->smem_y, st>>>(p->B, p->A, d, s.kz0, p->Wy, p->tw[1]); break;
-    case 5: p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]); break;
+    case 4: p4_y_inv_generic<<<dim3(d.nx / p->Wy, s.planes * nb), 256, p->smem_y, st>>>(p->B, p->A, d, s.kz0, p->Wy, p->tw[1]); break;
+    case 5: p5_z_c2r_generic<<<dim3(d.nx / (2 * p->Wz), d.ny, nb), 256, p->smem_z, st>>>(p->A, phi, d, p->Wz, p->tw[2]); break;
     }
 }
 
@@ -711,9 +713,13 @@ extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int co
     return n;
 }
 
-extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double *phi, void *stream)
+static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int nb, void *stream)
 {
     if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
+    if (nb < 1 || nb > p->max_batch)
+        return fail(DKS_ERR_INVALID_ARG, "batch of %d meshes: the plan is sized for at most %d (dks_poisson_set_max_batch)", nb, p->max_batch);
+    if (nb > 1 && (p->use_fused || p->slab != p->d.nz + 1))
+        return fail(DKS_ERR_INVALID_ARG, "batched solves need the default pipeline (no slabs, no fused kernel)");
     if ((reinterpret_cast<uintptr_t>(rho) | reinterpret_cast<uintptr_t>(phi)) % 16)
         return fail(DKS_ERR_INVALID_ARG, "rho and phi must be 16-byte aligned");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
@@ -747,11 +753,40 @@ extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double 
             DKS_FOR_EACH_FUSED(X)
 #undef X
             if (rc) return rc;
-        } else if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, st);
-        else launch_generic(s, p, rho, phi, st);
+        } else if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, nb, st);
+        else launch_generic(s, p, rho, phi, nb, st);
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
     DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_solve(dks_poisson_plan *p, const double *rho, double *phi, void *stream)
+{
+    return solve_impl(p, rho, phi, 1, stream);
+}
+
+extern "C" int dks_poisson_solve_batch(dks_poisson_plan *p, const double *rho, double *phi, int nbatch, void *stream)
+{
+    return solve_impl(p, rho, phi, nbatch, stream);
+}
+
+extern "C" int dks_poisson_set_max_batch(dks_poisson_plan *p, int nbatch)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (nbatch < 1 || nbatch > 64) return fail(DKS_ERR_INVALID_ARG, "nbatch must be in [1, 64]");
+    const int old = p->max_batch;
+    p->max_batch = nbatch;
+    compute_layout(p);
+    if (p->ws && p->ws_bytes < p->need_bytes) {
+        const size_t need = p->need_bytes;
+        p->max_batch = old;
+        compute_layout(p);
+        return fail(DKS_ERR_WORKSPACE_TOO_SMALL, "the attached workspace has %zu bytes, %zu needed for batches of %d; "
+                    "set the batch size before attaching the workspace / before dks_greens_setup", p->ws_bytes, need, nbatch);
+    }
+    p->prof_slots = 0;
+    if (p->ws) { bind_workspace(p); p->greens_ready = false; }      // the Green's octant moved
     return DKS_OK;
 }
 

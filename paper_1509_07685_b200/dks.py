@@ -28,6 +28,8 @@ SYMBOLS = {
     "dks_poisson_plan_destroy": (None, [_vp]),
     "dks_greens_setup": (_i, [_vp]),
     "dks_poisson_solve": (_i, [_vp, _vp, _vp, _vp]),
+    "dks_poisson_set_max_batch": (_i, [_vp, _i]),
+    "dks_poisson_solve_batch": (_i, [_vp, _vp, _vp, _i, _vp]),
     "dks_poisson_solve_host": (_i, [_vp, _vp, _vp, _vp]),
     "dks_poisson_solve_host_async": (_i, [_vp, _vp, _vp, _vp]),
     "dks_poisson_host_sync": (_i, [_vp]),
@@ -112,6 +114,15 @@ def dks_poisson_solve(plan, rho_dev, phi_dev, stream=None):
     return _check(lib.dks_poisson_solve(plan, _ptr(rho_dev), _ptr(phi_dev), stream), "dks_poisson_solve")
 
 
+def dks_poisson_set_max_batch(plan, nbatch):
+    return _check(lib.dks_poisson_set_max_batch(plan, int(nbatch)), "dks_poisson_set_max_batch")
+
+
+def dks_poisson_solve_batch(plan, rho_dev, phi_dev, nbatch, stream=None):
+    return _check(lib.dks_poisson_solve_batch(plan, _ptr(rho_dev), _ptr(phi_dev), int(nbatch), stream),
+                  "dks_poisson_solve_batch")
+
+
 def dks_poisson_solve_host(plan, rho_host, phi_host, stream=None):
     return _check(lib.dks_poisson_solve_host(plan, _ptr(rho_host), _ptr(phi_host), stream), "dks_poisson_solve_host")
 
@@ -193,7 +204,7 @@ def dks_poisson_copy_greens_hat(plan, host_out):
 class PoissonPlan:
     """Owns a dks_poisson_plan and a torch-allocated workspace on the current CUDA device."""
 
-    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, fused=None):
+    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, fused=None, max_batch=None):
         import torch
 
         self.n, self.h = tuple(int(v) for v in n), tuple(float(v) for v in h)
@@ -205,6 +216,8 @@ class PoissonPlan:
             dks_poisson_set_slab_planes(self._plan, slab_planes)
         if fused is not None:
             dks_poisson_set_fused(self._plan, fused)
+        if max_batch is not None:
+            dks_poisson_set_max_batch(self._plan, max_batch)
         if own_workspace:
             nbytes = dks_poisson_workspace_bytes(self._plan)
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
@@ -236,6 +249,20 @@ class PoissonPlan:
         elif not (phi.is_cuda and phi.dtype == torch.float64 and phi.is_contiguous() and phi.shape == rho.shape):
             raise ValueError("phi must match rho")
         dks_poisson_solve(self._plan, rho, phi, torch.cuda.current_stream().cuda_stream)
+        return phi
+
+    def solve_batch(self, rho, phi=None):
+        """rho, phi: CUDA float64 tensors of shape [nbatch, nz, ny, nx]; one launch per pass for the whole batch."""
+        import torch
+
+        nx, ny, nz = self.n
+        if not (rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous() and tuple(rho.shape[1:]) == (nz, ny, nx)):
+            raise ValueError(f"rho must be a contiguous CUDA float64 tensor of shape (nbatch, {nz}, {ny}, {nx})")
+        if phi is None:
+            phi = torch.empty_like(rho)
+        elif not (phi.is_cuda and phi.dtype == torch.float64 and phi.is_contiguous() and phi.shape == rho.shape):
+            raise ValueError("phi must match rho")
+        dks_poisson_solve_batch(self._plan, rho, phi, rho.shape[0], torch.cuda.current_stream().cuda_stream)
         return phi
 
     def solve_host(self, rho_host, phi_host):

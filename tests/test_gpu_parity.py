@@ -146,6 +146,28 @@ def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
     assert np.max(np.abs(g - direct) / np.abs(direct)) <= 1e-11
 
 
+# ---- batched solves: several meshes per launch, one Green's transform ------------------------------------
+@pytest.mark.parametrize("n,h", [((32, 16, 64), (2e-4, 3e-4, 1e-4)), ((64, 64, 64), (5e-4, 5e-4, 5e-4)),
+                                 ((8, 16, 8), (1e-3, 1e-3, 2e-3)), ((128, 32, 16), (1e-4, 2e-4, 4e-4))])
+def test_solve_batch_matches_single_solves_and_oracle(torch_cuda, dks, oracle, workloads, n, h):
+    torch = torch_cuda
+    nb = 3
+    rhos = np.stack([workloads.random_rho(n, seed=70 + i) for i in range(nb)])
+    plan = dks.PoissonPlan(n, h, max_batch=4)
+    try:
+        d = torch.from_numpy(rhos).cuda()
+        got = plan.solve_batch(d).cpu().numpy()
+        for i in range(nb):
+            single = plan.solve(d[i].contiguous()).cpu().numpy()
+            assert np.array_equal(got[i], single)           # same kernels, same arithmetic: bit-identical
+        check(got[1], oracle.solve(rhos[1], n, h, precision="ld"))
+        with pytest.raises(dks.DksError) as e:              # more meshes than the workspace was sized for
+            dks.dks_poisson_solve_batch(plan.handle, d, d, 5, None)
+        assert e.value.status == dks.DKS_ERR_INVALID_ARG
+    finally:
+        plan.close()
+
+
 # ---- opt-in variants: fused P2+P3+P4 cluster kernel (nx = 256, ny = 64..256) and slab-by-slab launches ----
 @pytest.mark.parametrize("n,h", [((256, 64, 8), (1e-4, 2e-4, 1e-3)), ((256, 128, 16), (1e-4, 1e-4, 4e-4)),
                                  ((256, 256, 40), (1e-4, 1e-4, 2e-4))])
