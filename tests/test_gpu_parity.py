@@ -274,6 +274,22 @@ def test_in_place_and_repeatable(torch_cuda, dks, oracle, workloads):
         plan.close()
 
 
+@pytest.mark.parametrize("n", [(128, 128, 128), (256, 64, 32), (64, 256, 256), (32, 16, 512)])
+def test_repeated_solves_are_bit_identical(torch_cuda, dks, workloads, n):
+    # races in the shared-memory exchanges / async prefetch pipelines would show up as run-to-run differences
+    torch = torch_cuda
+    plan = dks.PoissonPlan(n, (1e-4, 2e-4, 3e-4))
+    try:
+        d = torch.from_numpy(workloads.random_rho(n, seed=5)).cuda()
+        first = plan.solve(d).clone()
+        out = torch.empty_like(d)
+        for _ in range(40):
+            plan.solve(d, out)
+            assert torch.equal(out, first)
+    finally:
+        plan.close()
+
+
 def test_greens_hat_matches_oracle_transform(torch_cuda, dks, oracle):
     # Ghat octant (scale folded in) against numpy's FFT of the oracle-independent definition is NOT
     # used here; instead: solve of a unit point charge at the origin returns exactly G on the mesh.
