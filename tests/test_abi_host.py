@@ -93,3 +93,46 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert not pat.search(src), f"{f} reaches into oracle/"
+
+
+def test_host_only_plan_options(dks):
+    """Slab size, batch size and the fused switch are host-side plan state: workspace sizes and launch counts follow."""
+    nx, ny, nz = 256, 128, 64
+    p = dks.dks_poisson_plan_create(nx, ny, nz, 1e-4, 1e-4, 1e-4)
+    try:
+        a = 16 * nx * ny * (nz + 1)
+        ws1 = dks.dks_poisson_workspace_bytes(p)
+        assert dks.dks_poisson_slab_planes(p) == nz + 1 and dks.dks_poisson_launches_per_solve(p) == 5
+        # slabs of 13 planes: B shrinks to one slab, P2-P4 are launched once per slab
+        dks.dks_poisson_set_slab_planes(p, 13)
+        assert dks.dks_poisson_slab_planes(p) == 13
+        assert dks.dks_poisson_launches_per_solve(p) == 2 + 3 * 5
+        assert ws1 - dks.dks_poisson_workspace_bytes(p) >= 2 * a * (nz + 1 - 13) // (nz + 1) - 4096
+        dks.dks_poisson_set_slab_planes(p, 0)                                   # automatic again
+        assert dks.dks_poisson_workspace_bytes(p) == ws1
+        with pytest.raises(dks.DksError):
+            dks.dks_poisson_set_slab_planes(p, nz + 2)
+        # batches: A and B scale with the batch size
+        dks.dks_poisson_set_max_batch(p, 4)
+        assert dks.dks_poisson_workspace_bytes(p) - ws1 >= 3 * 3 * a - 4096
+        with pytest.raises(dks.DksError):
+            dks.dks_poisson_set_max_batch(p, 0)
+        dks.dks_poisson_set_max_batch(p, 1)
+        # fused P2+P3+P4 kernel: nx = 256 and ny in {64, 128, 256} only
+        assert dks.dks_poisson_fused(p) == 0
+        dks.dks_poisson_set_fused(p, 1)
+        assert dks.dks_poisson_fused(p) == 1 and dks.dks_poisson_launches_per_solve(p) == 3
+        assert dks.dks_poisson_pass_name(p, 3) == "p234_fused_r16"
+        dks.dks_poisson_set_fused(p, 0)
+        assert dks.dks_poisson_launches_per_solve(p) == 5
+    finally:
+        dks.dks_poisson_plan_destroy(p)
+    q = dks.dks_poisson_plan_create(128, 128, 128, 1e-4, 1e-4, 1e-4)
+    try:
+        with pytest.raises(dks.DksError) as e:
+            dks.dks_poisson_set_fused(q, 1)
+        assert e.value.status == dks.DKS_ERR_INVALID_ARG
+        assert [dks.dks_poisson_pass_name(q, i) for i in range(1, 6)] == [
+            "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"]
+    finally:
+        dks.dks_poisson_plan_destroy(q)
