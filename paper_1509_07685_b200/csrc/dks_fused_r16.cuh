@@ -17,9 +17,10 @@
 //
 // The arithmetic of every stage is that of the separate kernels (dks_passes_r16.cuh): the two
 // pruned length-n sub-transforms per padded line.  CTA = 512 threads = 512 / (16 A) column-tile teams
-// (named barriers) in S1/S3 and 16 line warps in S2; all twiddle tables live in shared memory (the L1
-// left beside 190 KB of shared memory is too small to hold them).  Scratch reads use ld.global.cg:
-// another SM wrote the data, so L1 must be bypassed.
+// (in lockstep behind __syncthreads) in S1/S3 and 16 line warps in S2; all twiddle tables live in shared
+// memory (the L1 left beside 185 KB of shared memory is too small to hold them).  Scratch reads use
+// ld.global.cg: another SM wrote the data, so L1 must be bypassed.
+// Opt-in (dks_poisson_set_fused): measured slower than the separate passes so far, DESIGN.md section 5.
 #pragma once
 #include "dks_passes_r16.cuh"
 
