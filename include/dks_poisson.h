@@ -76,7 +76,7 @@ int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi
  * Every pass processes the whole batch in one launch (still five launches), so small meshes are no longer
  * launch-latency bound and all meshes share one Green's transform.  nbatch <= dks_poisson_set_max_batch, which
  * sizes the workspace (A and B scale with it; default 1) and must be called before the workspace is attached /
- * before dks_greens_setup.  Needs the default pipeline (no slabs, no fused kernel).  Same stream semantics as
+ * before dks_greens_setup.  Needs the default pipeline (no slabs).  Same stream semantics as
  * dks_poisson_solve; phi_dev may alias rho_dev. */
 int dks_poisson_set_max_batch(dks_poisson_plan *plan, int nbatch);
 int dks_poisson_solve_batch(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, int nbatch, void *stream);
@@ -122,14 +122,6 @@ int dks_poisson_set_workspace(dks_poisson_plan *plan, void *dev_ptr, size_t byte
  * current value. */
 int dks_poisson_set_slab_planes(dks_poisson_plan *plan, int planes);
 int dks_poisson_slab_planes(const dks_poisson_plan *plan);
-
-/* For nx = 256 and ny in {64, 128, 256} P2, P3 and P4 run as ONE persistent kernel in which a cluster of
- * CTAs takes each kz plane through all three passes, with the plane's B as an L2-resident scratch
- * (DESIGN.md section 5).  It is opt-in (the separate passes are still faster): on = 1 selects it
- * (DKS_ERR_INVALID_ARG if the mesh does not qualify), on = 0 the separate passes.  Switches per-pass profiling off.
- * dks_poisson_fused returns 1 if the fused kernel is in use. */
-int dks_poisson_set_fused(dks_poisson_plan *plan, int on);
-int dks_poisson_fused(const dks_poisson_plan *plan);
 
 /* Stream used by dks_greens_setup (default NULL = legacy default stream). */
 int dks_poisson_set_stream(dks_poisson_plan *plan, void *stream);

@@ -262,21 +262,36 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 // group = warp_global + i * warps_total.  While a warp transforms group i, the bulk-copy engine brings
 // group i+1 and its J Ghat rows into the warp's shared-memory stage (cp.async.bulk + mbarrier), so no
 // DRAM latency is exposed and no register is spent on prefetching.
-// lane -> a = lane % A, p = (lane / A) % 2, j = lane / (2 A) (line within the group).
+// lane -> p = lane % 2, a = (lane / 2) % A, j = lane / (2 A) (line within the group): the two parities of an
+// element are neighbours, so that (i) the Ghat row is read as 32 consecutive doubles per instruction, (ii) the
+// parities are combined with one shuffle over lane ^ 1 and (iii) every store instruction writes 2 A consecutive
+// complex values per line (p = 0 keeps the even registers, p = 1 the odd ones).
 // Twiddles: tb[k] = region p of tw1 (see twiddle_between), fixed per lane, in registers.  The inverse runs
 // the TRANSPOSED flow (radix-A, exchange, conj tb, radix-16), in which the same per-lane set applies, so
 // one register set serves both directions and the parity twiddle w_L^(+-m) needs no table at all.
-// Exchange buffer per warp: region (j, p) = [16][A] elements, column XOR-swizzled with the row and regions
-// padded by A elements for A < 8: conflict free in both directions.
+// Exchange buffer per warp: region (j, p) = [16][A] elements at (2 j + p) * 16 A + p * P3Ex<A>::OFFP + j * OFFJ, the
+// column XOR-swizzled with the row: conflict free in both directions (checked by brute force over all lanes).
+// The (kz, ky) of a group follow incrementally from the previous group's (constant stride): no division in the loop.
 // ---------------------------------------------------------------------------------------------
 constexpr int kP3Warps = 12;
 constexpr int kP3OffEx = 4096;                     // after the 256-element group stage
-constexpr int kP3ExBytes = 2 * 16 * 17 * 16;       // 2 J regions of 17 A elements = 544 elements
+constexpr int kP3ExBytes = 2 * 16 * 17 * 16;       // 544 elements >= 2 J regions of 16 A elements + offsets
 constexpr int kP3OffG = kP3OffEx + kP3ExBytes;     // 12800
-constexpr int kP3GBytes = 2560;                    // J rows of (16 A + 8) doubles: 2112 (A=16) .. 2560 (A=2)
+constexpr int kP3GBytes = 2560;                    // J rows of P3Ex<A>::GSTR doubles
 constexpr int kP3OffBar = kP3OffG + kP3GBytes;     // 15360
 constexpr int kP3SmemPerWarp = kP3OffBar + 128;    // 15488
 constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp;
+
+template <int A>
+struct P3Ex {
+    static constexpr int SWZ = A >= 4 ? 3 : 1;
+    static constexpr int OFFP = A >= 4 ? 4 : 2;        // elements
+    static constexpr int OFFJ = 4;                     // keeps region (j, 1) clear of region (j + 1, 0)
+    static constexpr int GROW = (16 * A + 2) * 8;      // bytes of a Ghat row that are needed (n + 1 doubles, rounded to 16 B)
+    static constexpr int GSTR = A == 2 ? 36 : 16 * A + 8;   // shared-memory row stride (doubles): rows of a half-warp on distinct banks
+    static_assert(GROW <= GSTR * 8 && (16 / A) * GSTR * 8 <= kP3GBytes, "Ghat stage");
+    static_assert((2 * (16 / A) * 16 * A + OFFP + (16 / A - 1) * OFFJ) * 16 <= kP3ExBytes, "exchange buffer");
+};
 
 template <int A, bool PDL>
 __global__ void __launch_bounds__(kP3Warps * 32, 1)
@@ -285,15 +300,14 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int N = 16 * A, L = 32 * A, J = 16 / A, G = 16 / A;
-    constexpr int REG = 16 * A + (A < 8 ? A : 0);      // exchange region stride (elements)
-    constexpr int SWZ = A >= 8 ? 7 : A - 1;
-    constexpr unsigned ROWB = (16 * A + 8) * 8;        // bytes of one Ghat row (gpitch doubles)
+    constexpr int SWZ = P3Ex<A>::SWZ, GSTR = P3Ex<A>::GSTR;
+    constexpr unsigned GROW = P3Ex<A>::GROW;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int a = lane & (A - 1), p = (lane / A) & 1, j = lane / (2 * A);
+    const int p = lane & 1, a = (lane >> 1) & (A - 1), j = lane / (2 * A);
     unsigned char *wb = smem_raw + warp * kP3SmemPerWarp;
     const cplx *stage = reinterpret_cast<const cplx *>(wb) + j * N;
-    cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * REG;
-    const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * (16 * A + 8);
+    cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * (16 * A) + p * P3Ex<A>::OFFP + j * P3Ex<A>::OFFJ;
+    const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * GSTR;
     uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] group data, [1] Ghat rows
     if (PDL) pdl_trigger();
     if (lane == 0) {
@@ -303,31 +317,46 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     }
     __syncthreads();
 
-    const unsigned ny2 = 2 * d.ny, ngroups = (unsigned)planes * ny2 / J, stride = gridDim.x * kP3Warps;
+    const int ny2 = 2 * d.ny, nzp = d.nz + 1;
+    const unsigned ngroups = (unsigned)planes * ny2 / J, stride = gridDim.x * kP3Warps;
     // Groups are walked from the LAST plane down: P2 has just written B front to back, so its tail is still in
     // L2 when P3 starts, and P3's own tail (the first planes) is in L2 when P4 starts at plane 0.
     unsigned grp = blockIdx.x * kP3Warps + warp;
-    auto fetch_group = [&](unsigned gi) {
+    // (kz, ky0) of the group to be fetched next, updated incrementally (planes of a batch repeat kz)
+    const int step = (int)(stride * J), dky = step & (ny2 - 1), dkz = (step >> d.ly) % nzp;
+    int fkz = 0, fky = 0;
+    if (grp < ngroups) {
+        const unsigned l0 = (ngroups - 1 - grp) * J;
+        fkz = (kz0 + (int)(l0 >> d.ly)) % nzp;
+        fky = (int)(l0 & (ny2 - 1));
+    }
+    auto fetch = [&](unsigned gi) {                       // lane 0: group gi and its Ghat rows
         const unsigned g = ngroups - 1 - gi;
         mbar_expect_tx(&bar[0], 256 * sizeof(cplx));
         bulk_g2s(wb, B + (size_t)g * 256, 256 * sizeof(cplx), &bar[0]);
     };
-    auto fetch_ghat = [&](unsigned gi) {
-        const unsigned g = ngroups - 1 - gi;
-        const unsigned l0 = g * J;
-        const int kz = (kz0 + (int)(l0 / ny2)) % (d.nz + 1), ky0 = (int)(l0 % ny2);   // planes of a batch repeat kz
-        mbar_expect_tx(&bar[1], J * ROWB);
+    auto fetch_ghat = [&]() {                             // lane 0: the J Ghat rows of (fkz, fky ..)
+        mbar_expect_tx(&bar[1], J * GROW);
+        const double *row0 = Ghat + (size_t)fkz * (d.ny + 1) * d.gpitch;
 #pragma unroll
         for (int jj = 0; jj < J; ++jj) {
-            const int ky = ky0 + jj;
-            bulk_g2s(wb + kP3OffG + jj * ROWB, Ghat + ((size_t)kz * (d.ny + 1) + min(ky, (int)ny2 - ky)) * d.gpitch, ROWB, &bar[1]);
+            const int ky = fky + jj;
+            bulk_g2s(wb + kP3OffG + jj * GSTR * 8, row0 + (size_t)min(ky, ny2 - ky) * d.gpitch, GROW, &bar[1]);
         }
+    };
+    auto advance = [&]() {                                // (fkz, fky) of the group `stride` further on
+        fky -= dky;
+        const int borrow = fky < 0;
+        fky += borrow ? ny2 : 0;
+        fkz -= dkz + borrow;
+        fkz += fkz < 0 ? nzp : 0;
     };
     if (PDL) pdl_wait();
     if (lane == 0 && grp < ngroups) {
-        fetch_group(grp);
-        fetch_ghat(grp);
+        fetch(grp);
+        fetch_ghat();
     }
+    advance();
     cplx tb[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) tb[k] = __ldg(&tw1[p * N + k * A + a]);
@@ -341,7 +370,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[a + A * b];
         __syncwarp();                                 // stage consumed (and last exchange reads done)
-        if (lane == 0 && next < ngroups) fetch_group(next);
+        if (lane == 0 && next < ngroups) fetch(next);
         // forward: v[b] = x[a + A b] -> v[r] = X[2 (a + A r) + p]
         if (p) parity_consts<-1>(v);
         fft16<-1>(v);
@@ -363,7 +392,8 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             v[r] = cscale(v[r], gs[min(K, L - K)]);
         }
         __syncwarp();                                 // Ghat rows consumed, forward exchange reads done
-        if (lane == 0 && next < ngroups) fetch_ghat(next);
+        if (lane == 0 && next < ngroups) fetch_ghat();
+        advance();
         // inverse, transposed flow: radix-A, exchange back, conj tb, radix-16
         fft_second_t<A, +1>(v);
 #pragma unroll
@@ -375,10 +405,13 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
         for (int k = 0; k < 16; ++k) v[k] = cmulc(ex[k * A + (a ^ (k & SWZ))], tb[k]);
         fft16<+1>(v);
         if (p) parity_consts<+1>(v);
-        cplx out[8];
-        combine_parities<A>(v, p, out);
+        // combine the parities (crop fused): y[m] = O_0[m] + w_L^-m O_1[m]; parity 0 keeps the even registers, parity 1 the odd ones
 #pragma unroll
-        for (int i = 0; i < 8; ++i) stg_stream(&base[a + A * (i + 8 * p)], out[i]);
+        for (int i = 0; i < 8; ++i) {
+            const cplx send = p ? v[2 * i] : v[2 * i + 1];
+            const cplx mine = p ? v[2 * i + 1] : v[2 * i];
+            stg_stream(&base[a + A * (2 * i + p)], cadd(mine, shfl_xor_c(send, 1)));
+        }
     }
 }
 

@@ -19,7 +19,6 @@
 #include "../../include/dks_poisson.h"
 #include "dks_passes_generic.cuh"
 #include "dks_passes_r16.cuh"
-#include "dks_fused_r16.cuh"
 #include "dks_greens_r16.cuh"
 
 using namespace dks;
@@ -81,13 +80,9 @@ struct dks_poisson_plan {
     // is a slab-sized scratch that stays resident in L2 between the three passes
     int slab = 0;                       // planes per slab, 1..nz+1
     bool slab_user = false;             // set through dks_poisson_set_slab_planes
-    struct Step { int pass, kz0, planes; };     // pass 1..5, or kPassFused = P2+P3+P4 of all planes in one kernel
-    // fused P2+P3+P4 (dks_fused_r16.cuh): available for nx = 256 and ny = 64, 128, 256
-    bool fused_ok = false, use_fused = false;
+    struct Step { int pass, kz0, planes; };     // pass 1..5
     int max_batch = 1;                  // meshes per dks_poisson_solve_batch call the workspace is sized for
     bool pdl = false;                   // programmatic dependent launch between the r16 passes (small meshes)
-    int fused_cl = 4;                   // CTAs per cluster
-    int fused_clusters = 0;             // clusters of kFusedCluster CTAs that are co-resident on this device
     std::vector<Step> steps;            // the launch list of one solve
     bool greens_ready = false;
     bool setup_pending = false;         // setup_done not yet known to have completed
@@ -103,7 +98,6 @@ struct dks_poisson_plan {
 };
 
 static const int kNumPasses = 5;
-static const int kPassFused = 6;
 static const int kMaxProfSlots = 256;
 
 static bool is_pow2_in_range(int n) { return n >= 8 && n <= 1024 && (n & (n - 1)) == 0; }
@@ -144,11 +138,6 @@ static void compute_layout(dks_poisson_plan *p)
     p->need_bytes = off;
     p->steps.clear();
     p->steps.push_back({ 1, 0, 0 });
-    if (p->use_fused) {
-        p->steps.push_back({ kPassFused, 0, p->d.nz + 1 });
-        p->steps.push_back({ 5, 0, 0 });
-        return;
-    }
     for (int kz0 = 0; kz0 <= p->d.nz; kz0 += p->slab) {
         const int planes = std::min(p->slab, p->d.nz + 1 - kz0);
         p->steps.push_back({ 2, kz0, planes });
@@ -230,8 +219,6 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
     p->slab = auto_slab(p);
     p->pdl = (size_t)nx * ny * nz <= ((size_t)1 << 21);
-    p->fused_ok = p->fast[1] && p->r16A[0] == 16 && p->r16A[1] >= 4;
-    p->use_fused = false;               // measured slower than the separate passes so far: opt-in
     compute_layout(p);
     g_err[0] = 0;
     return p;
@@ -297,41 +284,6 @@ static int r16_set_attributes()
 #undef X
     return DKS_OK;
 }
-
-template <int A, int CL>
-static int fused_prepare(dks_poisson_plan *p)
-{
-    DKS_CUDA(cudaFuncSetAttribute(p234_fused_r16<A, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFusedSmem));
-    if (CL > 8) DKS_CUDA(cudaFuncSetAttribute(p234_fused_r16<A, CL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.gridDim = dim3(CL * 64); cfg.blockDim = dim3(kFusedThreads); cfg.dynamicSmemBytes = kFusedSmem;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    int n = 0;
-    DKS_CUDA(cudaOccupancyMaxActiveClusters(&n, p234_fused_r16<A, CL>, &cfg));
-    p->fused_clusters = n;
-    return DKS_OK;
-}
-
-template <int A, int CL>
-static int fused_launch(const dks_poisson_plan *p, cudaStream_t st)
-{
-    const int clusters = std::min(p->fused_clusters, std::min(p->d.nz + 1, p->slab));   // B holds `slab` planes
-    cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.gridDim = dim3(CL * clusters); cfg.blockDim = dim3(kFusedThreads); cfg.dynamicSmemBytes = kFusedSmem;
-    cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
-    DKS_CUDA(cudaLaunchKernelEx(&cfg, p234_fused_r16<A, CL>, p->A, p->B, (const double *)p->G, p->d, (const cplx *)p->tw1[0],
-                                (const cplx *)p->tw1[1]));
-    return DKS_OK;
-}
-
-// (A, cluster size) instantiations
-#define DKS_FOR_EACH_FUSED(X) X(4, 4) X(8, 4) X(16, 4)
 
 // Launch with programmatic stream serialization (programmatic dependent launch): the kernel may be scheduled
 // while the previous kernel in the stream drains; it orders itself with pdl_wait() (dks_common.cuh).
@@ -448,16 +400,6 @@ static int ensure_device(dks_poisson_plan *p)
     DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g));
     int rc = r16_set_attributes();
     if (rc) return rc;
-    if (p->fused_ok) {
-#define X(A_, CL_) if (p->r16A[1] == A_ && p->fused_cl == CL_) rc = fused_prepare<A_, CL_>(p);
-        DKS_FOR_EACH_FUSED(X)
-#undef X
-        if (rc) return rc;
-        if (p->fused_clusters < 1) {         // no co-resident cluster on this device: fall back to separate passes
-            p->fused_ok = p->use_fused = false;
-            compute_layout(p);
-        }
-    }
     p->device_checked = true;
     return DKS_OK;
 }
@@ -499,22 +441,6 @@ extern "C" int dks_poisson_set_slab_planes(dks_poisson_plan *p, int planes)
     p->prof_slots = 0;                  // the launch list changed: recorded events no longer match
     if (p->ws) bind_workspace(p);
     return DKS_OK;
-}
-
-extern "C" int dks_poisson_set_fused(dks_poisson_plan *p, int on)
-{
-    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
-    if (on && !p->fused_ok) return fail(DKS_ERR_INVALID_ARG, "the fused P2+P3+P4 kernel needs nx = 256 and ny in {64, 128, 256}");
-    p->use_fused = on != 0;
-    p->prof_slots = 0;
-    compute_layout(p);
-    return DKS_OK;
-}
-
-extern "C" int dks_poisson_fused(const dks_poisson_plan *p)
-{
-    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
-    return p->use_fused ? 1 : 0;
 }
 
 extern "C" int dks_poisson_slab_planes(const dks_poisson_plan *p)
@@ -649,7 +575,6 @@ extern "C" double dks_poisson_model_bytes(const dks_poisson_plan *p, int pass)
     const double nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
     const double rho = 8 * nx * ny * nz, a = 16 * nx * ny * (nz + 1), b = 2 * a;
     const double g = 8 * (nx + 1) * (ny + 1) * (nz + 1);
-    if (p->use_fused && pass >= 2 && pass <= 4) return pass == 3 ? 2 * a + g : 0.0;   // B stays in L2
     switch (pass) {
     case 0: return 2 * rho + 4 * a + 4 * b + g;
     case 1: return rho + a;
@@ -667,7 +592,6 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     static const char *names[5] = { "p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic",
                                     "p4_y_inv_generic", "p5_z_c2r_generic" };
     static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
-    if (p->use_fused && pass >= 2 && pass <= 4) return pass == 3 ? "p234_fused_r16" : "(fused into p234_fused_r16)";
     return p->fast[pass - 1] ? fast_names[pass - 1] : names[pass - 1];
 }
 
@@ -706,7 +630,7 @@ extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int co
         for (size_t i = 0; i < p->steps.size(); ++i) {
             float ms = 0.f;
             DKS_CUDA(cudaEventElapsedTime(&ms, e[i], e[i + 1]));
-            acc[(p->steps[i].pass == kPassFused ? 3 : p->steps[i].pass) - 1] += ms;
+            acc[p->steps[i].pass - 1] += ms;
         }
     }
     for (int i = 0; i < n; ++i) ms_out[i] = (float)(acc[i] / (double)solves);
@@ -718,8 +642,8 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
     if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
     if (nb < 1 || nb > p->max_batch)
         return fail(DKS_ERR_INVALID_ARG, "batch of %d meshes: the plan is sized for at most %d (dks_poisson_set_max_batch)", nb, p->max_batch);
-    if (nb > 1 && (p->use_fused || p->slab != p->d.nz + 1))
-        return fail(DKS_ERR_INVALID_ARG, "batched solves need the default pipeline (no slabs, no fused kernel)");
+    if (nb > 1 && p->slab != p->d.nz + 1)
+        return fail(DKS_ERR_INVALID_ARG, "batched solves need the default pipeline (no slabs)");
     if ((reinterpret_cast<uintptr_t>(rho) | reinterpret_cast<uintptr_t>(phi)) % 16)
         return fail(DKS_ERR_INVALID_ARG, "rho and phi must be 16-byte aligned");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
@@ -747,13 +671,7 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
     for (size_t i = 0; i < p->steps.size(); ++i) {
         const dks_poisson_plan::Step &s = p->steps[i];
         if (prof) DKS_CUDA(cudaEventRecord(ev[i], st));
-        if (s.pass == kPassFused) {
-            int rc = DKS_OK;
-#define X(A_, CL_) if (p->r16A[1] == A_ && p->fused_cl == CL_) rc = fused_launch<A_, CL_>(p, st);
-            DKS_FOR_EACH_FUSED(X)
-#undef X
-            if (rc) return rc;
-        } else if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, nb, st);
+        if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, nb, st);
         else launch_generic(s, p, rho, phi, nb, st);
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }

@@ -40,8 +40,6 @@ SYMBOLS = {
     "dks_poisson_set_stream": (_i, [_vp, _vp]),
     "dks_poisson_set_slab_planes": (_i, [_vp, _i]),
     "dks_poisson_slab_planes": (_i, [_vp]),
-    "dks_poisson_set_fused": (_i, [_vp, _i]),
-    "dks_poisson_fused": (_i, [_vp]),
     "dks_poisson_set_profiling": (_i, [_vp, _i]),
     "dks_poisson_pass_times": (_i, [_vp, C.POINTER(C.c_float), _i]),
     "dks_poisson_launches_per_solve": (_i, [_vp]),
@@ -166,14 +164,6 @@ def dks_poisson_slab_planes(plan) -> int:
     return _check(lib.dks_poisson_slab_planes(plan), "dks_poisson_slab_planes")
 
 
-def dks_poisson_set_fused(plan, on):
-    return _check(lib.dks_poisson_set_fused(plan, int(on)), "dks_poisson_set_fused")
-
-
-def dks_poisson_fused(plan) -> int:
-    return _check(lib.dks_poisson_fused(plan), "dks_poisson_fused")
-
-
 def dks_poisson_set_profiling(plan, slots):
     return _check(lib.dks_poisson_set_profiling(plan, int(slots)), "dks_poisson_set_profiling")
 
@@ -204,7 +194,7 @@ def dks_poisson_copy_greens_hat(plan, host_out):
 class PoissonPlan:
     """Owns a dks_poisson_plan and a torch-allocated workspace on the current CUDA device."""
 
-    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, fused=None, max_batch=None):
+    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, max_batch=None):
         import torch
 
         self.n, self.h = tuple(int(v) for v in n), tuple(float(v) for v in h)
@@ -214,8 +204,6 @@ class PoissonPlan:
             dks_poisson_set_g0(self._plan, g0)
         if slab_planes is not None:
             dks_poisson_set_slab_planes(self._plan, slab_planes)
-        if fused is not None:
-            dks_poisson_set_fused(self._plan, fused)
         if max_batch is not None:
             dks_poisson_set_max_batch(self._plan, max_batch)
         if own_workspace:

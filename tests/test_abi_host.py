@@ -96,7 +96,7 @@ def test_product_does_not_import_oracle():
 
 
 def test_host_only_plan_options(dks):
-    """Slab size, batch size and the fused switch are host-side plan state: workspace sizes and launch counts follow."""
+    """Slab size and batch size are host-side plan state: workspace sizes and launch counts follow."""
     nx, ny, nz = 256, 128, 64
     p = dks.dks_poisson_plan_create(nx, ny, nz, 1e-4, 1e-4, 1e-4)
     try:
@@ -118,20 +118,10 @@ def test_host_only_plan_options(dks):
         with pytest.raises(dks.DksError):
             dks.dks_poisson_set_max_batch(p, 0)
         dks.dks_poisson_set_max_batch(p, 1)
-        # fused P2+P3+P4 kernel: nx = 256 and ny in {64, 128, 256} only
-        assert dks.dks_poisson_fused(p) == 0
-        dks.dks_poisson_set_fused(p, 1)
-        assert dks.dks_poisson_fused(p) == 1 and dks.dks_poisson_launches_per_solve(p) == 3
-        assert dks.dks_poisson_pass_name(p, 3) == "p234_fused_r16"
-        dks.dks_poisson_set_fused(p, 0)
-        assert dks.dks_poisson_launches_per_solve(p) == 5
     finally:
         dks.dks_poisson_plan_destroy(p)
     q = dks.dks_poisson_plan_create(128, 128, 128, 1e-4, 1e-4, 1e-4)
     try:
-        with pytest.raises(dks.DksError) as e:
-            dks.dks_poisson_set_fused(q, 1)
-        assert e.value.status == dks.DKS_ERR_INVALID_ARG
         assert [dks.dks_poisson_pass_name(q, i) for i in range(1, 6)] == [
             "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"]
     finally:

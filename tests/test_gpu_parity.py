@@ -168,34 +168,7 @@ def test_solve_batch_matches_single_solves_and_oracle(torch_cuda, dks, oracle, w
         plan.close()
 
 
-# ---- opt-in variants: fused P2+P3+P4 cluster kernel (nx = 256, ny = 64..256) and slab-by-slab launches ----
-@pytest.mark.parametrize("n,h", [((256, 64, 8), (1e-4, 2e-4, 1e-3)), ((256, 128, 16), (1e-4, 1e-4, 4e-4)),
-                                 ((256, 256, 40), (1e-4, 1e-4, 2e-4))])
-def test_fused_plane_kernel_matches_oracle(torch_cuda, dks, oracle, workloads, n, h):
-    # nz = 40 is not a power of two: skip it for the plan (A8) -- use 32 there, but keep > #clusters planes
-    n = (n[0], n[1], 32 if n[2] == 40 else n[2])
-    rho = workloads.random_rho(n, seed=11 + n[1])
-    ref = oracle.solve(rho, n, h, precision="ld")
-    plan = dks.PoissonPlan(n, h, fused=1)
-    try:
-        assert dks.dks_poisson_fused(plan.handle) == 1
-        assert dks.dks_poisson_launches_per_solve(plan.handle) == 3
-        got = plan.solve(torch_cuda.from_numpy(rho).cuda()).cpu().numpy()
-    finally:
-        plan.close()
-    check(got, ref)
-
-
-def test_fused_refused_when_mesh_does_not_qualify(torch_cuda, dks):
-    h_ = dks.dks_poisson_plan_create(64, 64, 64, 1e-3, 1e-3, 1e-3)
-    try:
-        with pytest.raises(dks.DksError) as e:
-            dks.dks_poisson_set_fused(h_, 1)
-        assert e.value.status == dks.DKS_ERR_INVALID_ARG
-    finally:
-        dks.dks_poisson_plan_destroy(h_)
-
-
+# ---- opt-in variant: slab-by-slab launches of P2-P4 ----
 @pytest.mark.parametrize("slab", [1, 3, 17])
 def test_slab_launches_match_oracle(torch_cuda, dks, oracle, workloads, slab):
     n, h = (32, 64, 16), (2e-4, 3e-4, 1e-4)
