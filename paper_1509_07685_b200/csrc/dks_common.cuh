@@ -53,6 +53,12 @@ __device__ __forceinline__ void ldg_stream2(const cplx *p, cplx &v0, cplx &v1)
     asm volatile("ld.global.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v0.x), "=d"(v0.y), "=d"(v1.x), "=d"(v1.y) : "l"(p));
 }
 
+// the same through L1 (a second thread of the CTA reads the same 32 bytes shortly afterwards)
+__device__ __forceinline__ void ldg_cached2(const cplx *p, cplx &v0, cplx &v1)
+{
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v0.x), "=d"(v0.y), "=d"(v1.x), "=d"(v1.y) : "l"(p));
+}
+
 // Programmatic dependent launch (sm_90+).  Every pass kernel of the solve starts with pdl_trigger(): once all
 // CTAs of a grid have started, the next kernel in the stream may be scheduled into the SMs its tail frees
 // and run its prologue; pdl_wait() then blocks until the previous grid has completed and its memory is

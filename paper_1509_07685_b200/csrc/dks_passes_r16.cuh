@@ -132,13 +132,28 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
 // the packed spectrum C is split with FT{a}[k] = (C[k] + conj C[L-k]) / 2, FT{b}[k] = (C[k] - conj C[L-k]) / (2i).
 // Persistent: CTA t, t + grid, ... over the (nx / 16) * ny tiles of 16 real columns.  The next tile's
 // rho rows (N rows x 128 B) arrive in the shared-memory stage through cp.async while this tile is
-// transformed, so the DRAM latency is never exposed.  Split output: one 256-bit store per thread (FT{a}[k], FT{b}[k] are neighbours), 8 lanes = one 256-byte row.
+// transformed, so the DRAM latency is never exposed.
+// The split needs C[k] and C[L-k] in one thread.  After the transform, thread (a, p) holds C[2 (a + A r) + p] in
+// register r, and its mirror C[L-k] sits in register 15 - r of thread (A - a, 0) resp. (A - 1 - a, 1).  The a -> warp
+// map below puts every such pair of threads into one warp, 16 lanes apart (the self-paired a = 0 and a = A/2 of
+// parity 0 share warp 0), so the split is 8 register shuffles per value pair: no second pass through shared memory,
+// no further block barrier.  Each thread stores its 8 (9) rows k <= n as (FT{a}[k], FT{b}[k]) with one 256-bit
+// store (STG.256), 8 lanes = one 256-byte row.
 // ---------------------------------------------------------------------------------------------
 template <int A>
 struct P1Geom {
     static constexpr int STAGE = 16 * A * kCols * (int)sizeof(cplx);     // N rows x 8 packed pairs
     static constexpr int SMEM = R16Geom<A>::SMEM + STAGE;
 };
+
+// thread -> sub-transform index a such that mirror partners are lane ^ 16 (or the lane itself)
+template <int A>
+__device__ __forceinline__ int p1_a_of(int p, int s, int w)
+{
+    if (p) return s ? A - 1 - w : w;
+    if (w == 0) return s ? A / 2 : 0;
+    return s ? A - w : w;
+}
 
 template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
@@ -148,7 +163,10 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     extern __shared__ cplx ex[];
     constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
     cplx *stage = ex + L * kCols;
-    const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
+    const int tid = threadIdx.x, lane = tid & 31, c = tid & 7, p = (tid >> 3) & 1;
+    const int a = p1_a_of<A>(p, (tid >> 4) & 1, tid >> 5);
+    const bool a0 = a == 0 && p == 0;                     // holds k = 0 and k = n, mirrors inside its own registers
+    const int partner = (p == 0 && tid < 32) ? lane : lane ^ 16;
     const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny * nb;   // nb meshes back to back
     auto prefetch = [&](int t) {
         const int yy = t / xtiles, y = yy % ny;
@@ -169,10 +187,9 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     if (t < tiles) prefetch(t);
     for (; t < tiles; t += gridDim.x) {
         const int yy = t / xtiles, y = yy % ny;
-        cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx;
-        const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
+        cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx + (size_t)y * nx + (size_t)(t % xtiles) * 2 * kCols + 2 * c;
         cp_async_wait_all();
-        __syncthreads();                                  // stage complete; last tile's split reads done
+        __syncthreads();                                  // stage complete; last tile's exchange reads done
         cplx v[16];
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[(a + A * b) * kCols + c];
@@ -189,17 +206,17 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         for (int g = 0; g < G; ++g)
 #pragma unroll
             for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-        fft_second<A, -1>(v);
-        __syncthreads();                                  // exchange reads done: reuse ex as C[K][c]
+        fft_second<A, -1>(v);                             // v[r] = C[2 (a + A r) + p]
+        // ---- split: rows k = 2 (a + A r) + p, r < 8, and k = n (thread a0, r = 8)
 #pragma unroll
-        for (int r = 0; r < 16; ++r) ex[(2 * (a + A * r) + p) * kCols + c] = v[r];
-        __syncthreads();
-        for (int idx = tid; idx < (N + 1) * kCols; idx += THREADS) {
-            const int k = idx >> 3, cc = idx & 7;
-            const cplx ck = ex[k * kCols + cc], cm = ex[((L - k) & (L - 1)) * kCols + cc];
-            stg_stream2(&Aout[((size_t)k * ny + y) * nx + x0 + 2 * cc], cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
+        for (int r = 0; r < 8; ++r) {
+            cplx cm = cmake(__shfl_sync(0xffffffffu, v[15 - r].x, partner), __shfl_sync(0xffffffffu, v[15 - r].y, partner));
+            if (a0) cm = r == 0 ? v[0] : v[16 - r];
+            const cplx ck = v[r];
+            stg_stream2(Aout + (size_t)(2 * (a + A * r) + p) * ny * nx, cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
                         cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x)));
         }
+        if (a0) stg_stream2(Aout + (size_t)N * ny * nx, cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
     }
 }
 
@@ -273,7 +290,10 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 // column XOR-swizzled with the row: conflict free in both directions (checked by brute force over all lanes).
 // The (kz, ky) of a group follow incrementally from the previous group's (constant stride): no division in the loop.
 // ---------------------------------------------------------------------------------------------
-constexpr int kP3Warps = 12;
+#ifndef DKS_P3_WARPS
+#define DKS_P3_WARPS 12
+#endif
+constexpr int kP3Warps = DKS_P3_WARPS;
 constexpr int kP3OffEx = 4096;                     // after the 256-element group stage
 constexpr int kP3ExBytes = 2 * 16 * 17 * 16;       // 544 elements >= 2 J regions of 16 A elements + offsets
 constexpr int kP3OffG = kP3OffEx + kP3ExBytes;     // 12800

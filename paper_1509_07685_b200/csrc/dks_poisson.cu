@@ -2,7 +2,7 @@
 //
 // The plan owns: host metadata, device twiddle tables, profiling events, an ordering event between
 // dks_greens_setup and dks_poisson_solve, and (unless the caller attached one) the device workspace
-//     [ A | B | Ghat octant | host-path staging ].
+//     [ A | Ghat octant | host-path staging | B ].
 // dks_poisson_solve launches five kernels on the caller's stream and returns; it neither allocates
 // nor synchronises ("streams for asynchronous copy/compute").
 #include <algorithm>
@@ -88,6 +88,8 @@ struct dks_poisson_plan {
     bool setup_pending = false;         // setup_done not yet known to have completed
     cudaStream_t setup_stream = nullptr;
     cudaEvent_t setup_done = nullptr;
+    cudaEvent_t solve_done = nullptr;   // recorded after the last launch of a solve that runs on another stream than the setup
+    bool solve_recorded = false;
     // profiling
     int prof_slots = 0;                 // 0 = off; else per-pass events of the last prof_slots solves are kept
     long long prof_count = 0;           // profiled solves issued since profiling was switched on
@@ -239,7 +241,8 @@ static void release_device(dks_poisson_plan *p)
     if (p->ws_owned && p->ws) cudaFree(p->ws);
     p->ws = nullptr; p->ws_owned = false;
     if (p->setup_done) cudaEventDestroy(p->setup_done);
-    p->setup_done = nullptr;
+    if (p->solve_done) cudaEventDestroy(p->solve_done);
+    p->setup_done = p->solve_done = nullptr;
     for (int i = 0; i < 2; ++i) {
         if (p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
         if (p->ev_solve[i]) cudaEventDestroy(p->ev_solve[i]);
@@ -387,19 +390,27 @@ static int ensure_device(dks_poisson_plan *p)
         DKS_CUDA(cudaMemcpy(p->tw1[a], p->tw1_host[a].data(), bytes, cudaMemcpyHostToDevice));
     }
     DKS_CUDA(cudaEventCreateWithFlags(&p->setup_done, cudaEventDisableTiming));
-    const size_t smem_max = std::max(p->smem_x, std::max(p->smem_y, p->smem_z));
-    const size_t smem_g = (size_t)2 * std::max(p->d.nx, std::max(p->d.ny, p->d.nz)) * (4 + 1) * sizeof(cplx);
-    if ((size_t)prop.sharedMemPerBlockOptin < std::max(smem_max, smem_g))
-        return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device offers %zu B of shared memory per block, %zu needed",
-                    (size_t)prop.sharedMemPerBlockOptin, std::max(smem_max, smem_g));
-    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_z));
-    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_z));
-    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_y));
-    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_y));
-    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem_x));
-    DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g));
-    int rc = r16_set_attributes();
-    if (rc) return rc;
+    // cudaFuncAttributeMaxDynamicSharedMemorySize is a setter, not a running maximum, and the kernels are shared by all
+    // plans of the process: set every kernel once per device to the largest size any supported mesh needs (n = 1024).
+    static bool attributes_set[64] = {};
+    if (dev >= 64 || !attributes_set[dev]) {
+        const int kMaxL = 2048;
+        const size_t smem_strided = (size_t)kMaxL * tile_width_for(kMaxL) * sizeof(cplx);            // lines along y / z
+        const size_t smem_lines = (size_t)kMaxL * (tile_width_for(kMaxL) + 1) * sizeof(cplx);        // lines along x, Green's axes
+        if ((size_t)prop.sharedMemPerBlockOptin < smem_lines)
+            return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device offers %zu B of shared memory per block, %zu needed",
+                        (size_t)prop.sharedMemPerBlockOptin, smem_lines);
+        DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_strided));
+        DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_strided));
+        DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_strided));
+        DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_strided));
+        DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_lines));
+        DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_lines));
+        int rc = r16_set_attributes();
+        if (rc) return rc;
+        if (dev < 64) attributes_set[dev] = true;
+    }
+    DKS_CUDA(cudaEventCreateWithFlags(&p->solve_done, cudaEventDisableTiming));
     p->device_checked = true;
     return DKS_OK;
 }
@@ -490,6 +501,8 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
     }
     const MeshDims d = p->d;
     cudaStream_t st = p->setup_stream;
+    // the rebuild overwrites Ghat: order it after the last solve issued on another stream (P3 reads Ghat)
+    if (p->solve_recorded) DKS_CUDA(cudaStreamWaitEvent(st, p->solve_done, 0));
     // 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), evaluated in long double.
     const long double pi_l = 3.141592653589793238462643383279502884L;
     const double coef = (double)(1.0L / (4.0L * pi_l * 8.8541878128e-12L));
@@ -648,12 +661,13 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
         return fail(DKS_ERR_INVALID_ARG, "rho and phi must be 16-byte aligned");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (p->setup_pending || st != p->setup_stream) DKS_CUDA(cudaStreamIsCapturing(st, &cs));
+    const bool capturing = cs != cudaStreamCaptureStatusNone;   // graph replays are ordered against dks_greens_setup by the caller
     if (p->setup_pending) {
         // Order this solve after the Green's setup.  A stream under capture must not wait on work
         // recorded outside the capture, so there the host waits for the setup instead (once).
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        DKS_CUDA(cudaStreamIsCapturing(st, &cs));
-        if (cs != cudaStreamCaptureStatusNone) {
+        if (capturing) {
             cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
             DKS_CUDA(cudaThreadExchangeStreamCaptureMode(&mode));
             cudaError_t e = cudaEventSynchronize(p->setup_done);
@@ -676,6 +690,10 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
     DKS_CUDA(cudaGetLastError());
+    if (st != p->setup_stream && !capturing) {          // a later dks_greens_setup on the setup stream must not overtake this solve
+        DKS_CUDA(cudaEventRecord(p->solve_done, st));
+        p->solve_recorded = true;
+    }
     return DKS_OK;
 }
 
@@ -693,6 +711,8 @@ extern "C" int dks_poisson_set_max_batch(dks_poisson_plan *p, int nbatch)
 {
     if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
     if (nbatch < 1 || nbatch > 64) return fail(DKS_ERR_INVALID_ARG, "nbatch must be in [1, 64]");
+    if ((long long)(p->d.nz + 1) * nbatch > 65535)      // P2 / P4 put (plane, mesh) on gridDim.y
+        return fail(DKS_ERR_INVALID_ARG, "(nz + 1) * nbatch = %lld exceeds 65535 (grid limit of the y passes)", (long long)(p->d.nz + 1) * nbatch);
     const int old = p->max_batch;
     p->max_batch = nbatch;
     compute_layout(p);
