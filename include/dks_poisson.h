@@ -40,7 +40,6 @@ typedef enum dks_status {
     DKS_OK = 0,
     DKS_ERR_INVALID_ARG = -1,        /* NULL pointer, n not a power of two in [8,1024], h <= 0 or not finite */
     DKS_ERR_UNSUPPORTED_DEVICE = -2, /* current device is not compute capability 10.x                      */
-    DKS_ERR_NO_WORKSPACE = -3,       /* (reserved)                                                         */
     DKS_ERR_WORKSPACE_TOO_SMALL = -4,/* dks_poisson_set_workspace: bytes < dks_poisson_workspace_bytes     */
     DKS_ERR_NOT_SETUP = -5,          /* dks_poisson_solve before dks_greens_setup (or after a spacing change) */
     DKS_ERR_CUDA = -6                /* a CUDA runtime call failed; see dks_last_error()                   */
@@ -48,12 +47,15 @@ typedef enum dks_status {
 
 typedef struct dks_poisson_plan dks_poisson_plan;   /* opaque */
 
-/* Creates a plan for an nx x ny x nz mesh with spacings hx, hy, hz [m].  Host-only: validates the
+/* Creates a plan for an nx x ny x nz mesh (the paper's Mx x My x Mz) with spacings hx, hy, hz [m]
+ * (the mesh is fitted to the bunch, so h is a per-time-step quantity).  The plan plays the role of the
+ * device-side state that DKS keeps between the calls of Fig. 2.  Host-only: validates the
  * arguments and computes the twiddle tables on the host; touches no device.  Returns NULL on
  * failure (dks_last_error() says why). */
 dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, double hx, double hy, double hz);
 
-/* Frees the plan, its device tables and (if plan-owned) its workspace.  NULL is allowed. */
+/* Frees the plan, its device tables and (if plan-owned) its workspace (Fig. 2's freeMemory).  Caller-owned
+ * workspaces are left alone.  The caller makes sure no solve of this plan is still running.  NULL is allowed. */
 void dks_poisson_plan_destroy(dks_poisson_plan *plan);
 
 /* Step a0 ("separate kernels to calculate the Greens function"):
@@ -67,8 +69,10 @@ int dks_greens_setup(dks_poisson_plan *plan);
 /* The hot path: phi = hx hy hz FT^-1{FT{rho} (x) FT{G}} cropped to the mesh.
  * rho_dev, phi_dev: device pointers as described above; rho_dev is only read; phi_dev may alias
  * rho_dev.  stream: a cudaStream_t (NULL = legacy default stream).  Asynchronous and stream-ordered:
- * no host synchronisation, no allocation; CUDA-graph capturable.  Launches P1, then P2-P3-P4 once per
- * slab of kz planes (dks_poisson_set_slab_planes), then P5: 2 + 3 * ceil((nz+1)/slab) kernels. */
+ * no host synchronisation, no allocation; CUDA-graph capturable (a captured solve is not ordered against later
+ * dks_greens_setup calls: the caller orders graph replays and rebuilds).  Launches P1, then P2-P3-P4 once per
+ * slab of kz planes (dks_poisson_set_slab_planes; default: one slab), then P5: 2 + 3 * ceil((nz+1)/slab) kernels.
+ * Errors: DKS_ERR_INVALID_ARG (NULL or misaligned pointer), DKS_ERR_NOT_SETUP, DKS_ERR_CUDA. */
 int dks_poisson_solve(dks_poisson_plan *plan, const double *rho_dev, double *phi_dev, void *stream);
 
 /* Several independent meshes of the same shape and spacing in one call (e.g. neighbouring bunches, PAPER.md:140
@@ -83,8 +87,10 @@ int dks_poisson_solve_batch(dks_poisson_plan *plan, const double *rho_dev, doubl
 
 /* Same solve with HOST buffers (the end-to-end path of the paper: rho is copied to
  * the device and phi back every step).  rho_host/phi_host: host pointers ([nz][ny][nx] fp64; pinned
- * memory recommended).  Copies H2D, solves, copies D2H on `stream`, then synchronises the stream.
- * The staging buffer is part of the workspace. */
+ * memory recommended).  = dks_poisson_solve_host_async followed by dks_poisson_host_sync: the copies run on
+ * plan-owned streams, the solve on `stream`, and the call returns when phi_host is complete.  Work issued on
+ * `stream` afterwards is ordered after the solve, not after the copy-out (the host has waited for that).
+ * The staging buffers are part of the workspace. */
 int dks_poisson_solve_host(dks_poisson_plan *plan, const double *rho_host, double *phi_host, void *stream);
 
 /* The same without the final synchronisation, so that consecutive steps overlap (PAPER.md:132 overlaps the rho
@@ -96,34 +102,50 @@ int dks_poisson_solve_host(dks_poisson_plan *plan, const double *rho_host, doubl
 int dks_poisson_solve_host_async(dks_poisson_plan *plan, const double *rho_host, double *phi_host, void *stream);
 int dks_poisson_host_sync(dks_poisson_plan *plan);
 
-/* Changes the mesh spacings (they are time dependent).  Invalidates the Green's
- * transform: call dks_greens_setup again before the next solve. */
+/* One time step exactly as the paper runs it (Fig. 5: "CUDA streams are used to overlap the transfer of
+ * the rho field to the GPU and the calculation of the Greens function"; the spacings change every step):
+ * dks_poisson_set_spacing(hx, hy, hz), then the Green's rebuild (step a0) on the setup stream -- a plan-owned stream
+ * unless dks_poisson_set_stream gave one that differs from `stream` -- concurrently with the host-to-device copy of
+ * rho on the copy-in stream; the solve on `stream` waits for both, the copy-out follows on the copy-out stream.  The
+ * rebuild of step i+1 is ordered after P3 of step i (the only reader of the Green's transform), so it also overlaps
+ * P4, P5 and the copy-out of step i.  Same buffer rules as dks_poisson_solve_host_async; finish with
+ * dks_poisson_host_sync. */
+int dks_poisson_step_host_async(dks_poisson_plan *plan, double hx, double hy, double hz, const double *rho_host,
+                                double *phi_host, void *stream);
+
+/* Changes the mesh spacings (they are time dependent).  Host-only.  Invalidates the Green's
+ * transform: call dks_greens_setup again before the next solve (DKS_ERR_NOT_SETUP otherwise). */
 int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double hz);
 
-/* Overrides G(0,0,0); NaN restores the default rule.  Invalidates the Green's transform. */
+/* Overrides G(0,0,0), which PAPER.md:117 leaves undefined (G = 1/r is singular there; reading A2);
+ * NaN restores the default rule G(r0), r0 = min(hx,hy,hz)/2.  Host-only.  Invalidates the Green's transform. */
 int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
 
 /* Bytes of device workspace the plan needs (buffer A, the Green's octant, the two host-path staging
- * meshes, one slab of B). */
+ * meshes, one slab of B).  "Memory management is left up to the user": the caller may allocate it
+ * (Fig. 2's allocateMemory) and attach it with dks_poisson_set_workspace.  Host-only. */
 size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
 
-/* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace; 256-byte aligned,
- * at least dks_poisson_workspace_bytes().  The caller keeps ownership and must keep it alive.
- * Invalidates the Green's transform. */
+/* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace (Fig. 2);
+ * 256-byte aligned, at least dks_poisson_workspace_bytes() (else DKS_ERR_WORKSPACE_TOO_SMALL).  The caller keeps
+ * ownership and must keep it alive.  Invalidates the Green's transform.  Without it dks_greens_setup allocates a
+ * plan-owned workspace on first use. */
 int dks_poisson_set_workspace(dks_poisson_plan *plan, void *dev_ptr, size_t bytes);
 
 /* P2, P3 and P4 work on independent kz planes of the half-spectrum (kz = 0..nz).  They are launched
  * slab by slab -- `planes` consecutive kz planes at a time -- so that the buffer B between them
  * ([planes][2ny][nx] complex) is a scratch that stays in the L2 cache instead of going through HBM.
- * planes = 0 restores the automatic choice (about 40 MB of B per slab); planes = nz+1 is the unslabbed
- * pipeline.  Changes dks_poisson_workspace_bytes(); call it before attaching a workspace / before
+ * planes = 0 restores the automatic choice, which is one slab of all nz+1 planes (measured: every slab boundary
+ * costs more than the L2 residency saves); planes = nz+1 is the same unslabbed pipeline.  Changes dks_poisson_workspace_bytes(); call it before attaching a workspace / before
  * dks_greens_setup (afterwards it fails with DKS_ERR_WORKSPACE_TOO_SMALL if the workspace cannot
  * hold the new slab).  Switches per-pass profiling off.  dks_poisson_slab_planes returns the
  * current value. */
 int dks_poisson_set_slab_planes(dks_poisson_plan *plan, int planes);
 int dks_poisson_slab_planes(const dks_poisson_plan *plan);
 
-/* Stream used by dks_greens_setup (default NULL = legacy default stream). */
+/* Stream used by dks_greens_setup (default NULL = legacy default stream): "GPU streams are used" for asynchronous
+ * work, here to overlap the Green's rebuild with the rho transfer.  Solves on other
+ * streams are ordered after the rebuild, and the next rebuild after their P3, by plan-owned events.  Host-only. */
 int dks_poisson_set_stream(dks_poisson_plan *plan, void *stream);
 
 /* Per-pass timing.  slots > 0: dks_poisson_solve records CUDA events on its stream around each of
@@ -144,7 +166,9 @@ const char *dks_poisson_pass_name(const dks_poisson_plan *plan, int pass); /* ke
  * (nx+1)(ny+1)(nz+1) doubles; synchronises.  For tests. */
 int dks_poisson_copy_greens_hat(dks_poisson_plan *plan, double *host_out);
 
-/* Thread-local message describing the last error in this thread ("" if none). */
+/* Thread-local, NUL-terminated message describing the last failure in this thread ("" if none).  The library never
+ * throws or aborts: every entry point reports through its status (the paper's DKS layer hands device errors back to
+ * the host application in the same way). */
 const char *dks_last_error(void);
 
 #ifdef __cplusplus

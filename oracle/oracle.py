@@ -35,6 +35,7 @@ def _lib(precision: str):
         f = getattr(lib, p + "plan_destroy"); f.argtypes = [C.c_void_p]; f.restype = None
         f = getattr(lib, p + "plan_ghat_stats"); f.argtypes = [C.c_void_p, dp, dp, dp]; f.restype = None
         f = getattr(lib, p + "plan_solve"); f.argtypes = [C.c_void_p, dp, dp]; f.restype = C.c_double
+        f = getattr(lib, p + "plan_ghat_octant"); f.argtypes = [C.c_void_p, dp]; f.restype = None
         f = getattr(lib, p + "solve")
         f.argtypes = [C.c_int] * 3 + [C.c_double] * 5 + [dp, dp]; f.restype = C.c_double
         f = getattr(lib, p + "direct_sum_nodes")
@@ -94,6 +95,13 @@ class Plan:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         getattr(self._lib, self._p + "plan_ghat_stats")(self._h, C.byref(a), C.byref(b), C.byref(c))
         return {"max_im": a.value, "max_abs": b.value, "max_even_defect": c.value}
+
+    def ghat_octant(self):
+        """Re FT{Gt} on the octant [nz+1][ny+1][nx+1] (unscaled: no hx hy hz, no 1/N)."""
+        nx, ny, nz = self.n
+        out = np.empty((nz + 1, ny + 1, nx + 1), dtype=np.float64)
+        getattr(self._lib, self._p + "plan_ghat_octant")(self._h, _dp(out))
+        return out
 
     def close(self):
         if self._h:

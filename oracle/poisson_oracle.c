@@ -261,6 +261,17 @@ void FN(plan_ghat_stats)(void *vp, double *max_im, double *max_abs, double *max_
     *max_im = (double)mi; *max_abs = (double)ma; *max_even_defect = (double)me;
 }
 
+/* Accessor (no arithmetic): Re FT{Gt}[k][j][i] on the octant k <= nz, j <= ny, i <= nx of the doubled grid, as
+ * [nz+1][ny+1][nx+1] doubles.  FT{Gt} is real and even (pin P8), so the octant carries the whole transform; tests
+ * compare the CUDA path's Green's octant (step a0) with this directly. */
+void FN(plan_ghat_octant)(void *vp, double *out)
+{
+    oracle_plan *p = (oracle_plan *)vp;
+    size_t X = 2 * (size_t)p->nx, Y = 2 * (size_t)p->ny;
+    for (int k = 0; k <= p->nz; ++k) for (int j = 0; j <= p->ny; ++j) for (int i = 0; i <= p->nx; ++i)
+        out[((size_t)k * (p->ny + 1) + j) * (p->nx + 1) + i] = (double)p->Ghat[((size_t)k * Y + j) * X + i].re;
+}
+
 /* Steps 1, 3 (rho), 4, 5, 6.  rho, phi: [nz][ny][nx] doubles, x fastest.  Returns max |Im R| over the
  * low corner after step 5, relative to max |Re R| there (0 if phi == 0). */
 double FN(plan_solve)(void *vp, const double *rho, double *phi)

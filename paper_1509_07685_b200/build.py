@@ -41,13 +41,20 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
+    import fcntl
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE] + SOURCES + ["-o", LIB]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or r.returncode:
-        sys.stderr.write(r.stdout + r.stderr)
-    if r.returncode:
-        raise RuntimeError("nvcc failed building libdks_poisson.so")
+    with open(LIB + ".lock", "w") as lock:             # several ranks may import the package at once
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not stale():                  # another process built it while this one waited
+            return LIB
+        tmp = f"{LIB}.{os.getpid()}.tmp"
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE] + SOURCES + ["-o", tmp]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or r.returncode:
+            sys.stderr.write(r.stdout + r.stderr)
+        if r.returncode:
+            raise RuntimeError("nvcc failed building libdks_poisson.so")
+        os.replace(tmp, LIB)                           # atomic: no process ever maps a half-written library
     return LIB
 
 

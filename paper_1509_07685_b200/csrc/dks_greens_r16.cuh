@@ -12,8 +12,9 @@
 //                        pairs of octant rows (ky, ky + 1), the structure of p3_x_conv_r16's forward half.
 //   greens_axis_r16<A> : y or z axis, in place on the octant: the structure of p2_y_fwd_r16; a CTA takes 16
 //                        adjacent x entries (8 packed pairs) of all n + 1 rows along the axis.
-// The pad entries nx < kx < gpitch of every octant row are kept at zero: they are the imaginary partners
-// of valid columns in the packed strided passes and must stay finite.
+// The pad entries nx < kx < gpitch of every octant row are written as zero by the x pass: they are the imaginary
+// partners of valid columns in the packed y / z passes and must stay finite (entry nx + 1, the partner of column nx,
+// picks up that column's rounding leakage, ~1e-16 of it; P3 never reads a pad entry).
 #pragma once
 #include "dks_passes_r16.cuh"
 

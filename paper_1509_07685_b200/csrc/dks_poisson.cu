@@ -86,10 +86,12 @@ struct dks_poisson_plan {
     std::vector<Step> steps;            // the launch list of one solve
     bool greens_ready = false;
     bool setup_pending = false;         // setup_done not yet known to have completed
-    cudaStream_t setup_stream = nullptr;
+    cudaStream_t setup_stream = nullptr;   // stream dks_greens_setup launches on (dks_poisson_set_stream)
+    cudaStream_t setup_used = nullptr;     // stream the current Ghat was built on
+    cudaStream_t s_setup = nullptr;        // plan-owned stream of dks_poisson_step_host_async's rebuild
     cudaEvent_t setup_done = nullptr;
-    cudaEvent_t solve_done = nullptr;   // recorded after the last launch of a solve that runs on another stream than the setup
-    bool solve_recorded = false;
+    cudaEvent_t ghat_free = nullptr;    // recorded after the last P3 of a solve that runs on another stream than the setup:
+    bool ghat_free_recorded = false;    // the next rebuild of Ghat waits for it
     // profiling
     int prof_slots = 0;                 // 0 = off; else per-pass events of the last prof_slots solves are kept
     long long prof_count = 0;           // profiled solves issued since profiling was switched on
@@ -241,8 +243,10 @@ static void release_device(dks_poisson_plan *p)
     if (p->ws_owned && p->ws) cudaFree(p->ws);
     p->ws = nullptr; p->ws_owned = false;
     if (p->setup_done) cudaEventDestroy(p->setup_done);
-    if (p->solve_done) cudaEventDestroy(p->solve_done);
-    p->setup_done = p->solve_done = nullptr;
+    if (p->ghat_free) cudaEventDestroy(p->ghat_free);
+    p->setup_done = p->ghat_free = nullptr;
+    if (p->s_setup) cudaStreamDestroy(p->s_setup);
+    p->s_setup = nullptr;
     for (int i = 0; i < 2; ++i) {
         if (p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
         if (p->ev_solve[i]) cudaEventDestroy(p->ev_solve[i]);
@@ -410,7 +414,7 @@ static int ensure_device(dks_poisson_plan *p)
         if (rc) return rc;
         if (dev < 64) attributes_set[dev] = true;
     }
-    DKS_CUDA(cudaEventCreateWithFlags(&p->solve_done, cudaEventDisableTiming));
+    DKS_CUDA(cudaEventCreateWithFlags(&p->ghat_free, cudaEventDisableTiming));
     p->device_checked = true;
     return DKS_OK;
 }
@@ -489,9 +493,8 @@ extern "C" int dks_poisson_set_g0(dks_poisson_plan *p, double g0)
 // ------------------------------------------------------------------------------------------------
 // a0: Green's function build + transform
 // ------------------------------------------------------------------------------------------------
-extern "C" int dks_greens_setup(dks_poisson_plan *p)
+static int greens_setup_on(dks_poisson_plan *p, cudaStream_t st)
 {
-    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
     int rc = ensure_device(p);
     if (rc) return rc;
     if (!p->ws) {
@@ -500,9 +503,8 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
         bind_workspace(p);
     }
     const MeshDims d = p->d;
-    cudaStream_t st = p->setup_stream;
-    // the rebuild overwrites Ghat: order it after the last solve issued on another stream (P3 reads Ghat)
-    if (p->solve_recorded) DKS_CUDA(cudaStreamWaitEvent(st, p->solve_done, 0));
+    // the rebuild overwrites Ghat: order it after the last P3 issued on another stream (P3 is the only reader of Ghat)
+    if (p->ghat_free_recorded) DKS_CUDA(cudaStreamWaitEvent(st, p->ghat_free, 0));
     // 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), evaluated in long double.
     const long double pi_l = 3.141592653589793238462643383279502884L;
     const double coef = (double)(1.0L / (4.0L * pi_l * 8.8541878128e-12L));
@@ -559,7 +561,14 @@ extern "C" int dks_greens_setup(dks_poisson_plan *p)
     DKS_CUDA(cudaEventRecord(p->setup_done, st));
     p->greens_ready = true;
     p->setup_pending = true;
+    p->setup_used = st;
     return DKS_OK;
+}
+
+extern "C" int dks_greens_setup(dks_poisson_plan *p)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    return greens_setup_on(p, p->setup_stream);
 }
 
 extern "C" int dks_poisson_copy_greens_hat(dks_poisson_plan *p, double *host_out)
@@ -650,6 +659,12 @@ extern "C" int dks_poisson_pass_times(dks_poisson_plan *p, float *ms_out, int co
     return n;
 }
 
+static bool last_p3(const dks_poisson_plan *p, size_t i)
+{
+    for (size_t j = i + 1; j < p->steps.size(); ++j) if (p->steps[j].pass == 3) return false;
+    return true;
+}
+
 static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int nb, void *stream)
 {
     if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
@@ -662,7 +677,7 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-    if (p->setup_pending || st != p->setup_stream) DKS_CUDA(cudaStreamIsCapturing(st, &cs));
+    if (p->setup_pending || st != p->setup_used) DKS_CUDA(cudaStreamIsCapturing(st, &cs));
     const bool capturing = cs != cudaStreamCaptureStatusNone;   // graph replays are ordered against dks_greens_setup by the caller
     if (p->setup_pending) {
         // Order this solve after the Green's setup.  A stream under capture must not wait on work
@@ -675,7 +690,7 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
             DKS_CUDA(e);
             p->setup_pending = false;
         } else {
-            if (st != p->setup_stream) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+            if (st != p->setup_used) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
             if (cudaEventQuery(p->setup_done) == cudaSuccess) p->setup_pending = false;
             else (void)cudaGetLastError();   // cudaErrorNotReady is not a failure
         }
@@ -687,13 +702,14 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
         if (prof) DKS_CUDA(cudaEventRecord(ev[i], st));
         if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, nb, st);
         else launch_generic(s, p, rho, phi, nb, st);
+        // a later rebuild of Ghat on the setup stream must not overtake this solve's last P3
+        if (s.pass == 3 && last_p3(p, i) && st != p->setup_used && !capturing) {
+            DKS_CUDA(cudaEventRecord(p->ghat_free, st));
+            p->ghat_free_recorded = true;
+        }
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
     DKS_CUDA(cudaGetLastError());
-    if (st != p->setup_stream && !capturing) {          // a later dks_greens_setup on the setup stream must not overtake this solve
-        DKS_CUDA(cudaEventRecord(p->solve_done, st));
-        p->solve_recorded = true;
-    }
     return DKS_OK;
 }
 
@@ -760,6 +776,24 @@ extern "C" int dks_poisson_solve_host_async(dks_poisson_plan *p, const double *r
     DKS_CUDA(cudaEventRecord(p->ev_out[slot], p->s_out));
     // later work on the caller's stream is ordered after this call's copy-out only through dks_poisson_host_sync
     return DKS_OK;
+}
+
+// One OPAL time step as PAPER.md:132 runs it: the spacings change every step, so the Green's function is
+// rebuilt, on its own stream, while rho is still on its way to the device; the solve waits for both.
+extern "C" int dks_poisson_step_host_async(dks_poisson_plan *p, double hx, double hy, double hz, const double *rho_host,
+                                           double *phi_host, void *stream)
+{
+    if (!p || !rho_host || !phi_host) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
+    int rc = dks_poisson_set_spacing(p, hx, hy, hz);
+    if (rc) return rc;
+    cudaStream_t ss = p->setup_stream;
+    if (!ss || ss == static_cast<cudaStream_t>(stream)) {          // no stream of its own was given: use a plan-owned one
+        if (!p->s_setup) DKS_CUDA(cudaStreamCreateWithFlags(&p->s_setup, cudaStreamNonBlocking));
+        ss = p->s_setup;
+    }
+    rc = greens_setup_on(p, ss);                                    // waits for the previous step's P3, not for its P4 / P5 / copy-out
+    if (rc) return rc;
+    return dks_poisson_solve_host_async(p, rho_host, phi_host, stream);   // H2D on the copy stream; the solve waits for both
 }
 
 extern "C" int dks_poisson_host_sync(dks_poisson_plan *p)

@@ -16,7 +16,6 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 DKS_OK = 0
 DKS_ERR_INVALID_ARG = -1
 DKS_ERR_UNSUPPORTED_DEVICE = -2
-DKS_ERR_NO_WORKSPACE = -3
 DKS_ERR_WORKSPACE_TOO_SMALL = -4
 DKS_ERR_NOT_SETUP = -5
 DKS_ERR_CUDA = -6
@@ -33,6 +32,7 @@ SYMBOLS = {
     "dks_poisson_solve_host": (_i, [_vp, _vp, _vp, _vp]),
     "dks_poisson_solve_host_async": (_i, [_vp, _vp, _vp, _vp]),
     "dks_poisson_host_sync": (_i, [_vp]),
+    "dks_poisson_step_host_async": (_i, [_vp, _d, _d, _d, _vp, _vp, _vp]),
     "dks_poisson_set_spacing": (_i, [_vp, _d, _d, _d]),
     "dks_poisson_set_g0": (_i, [_vp, _d]),
     "dks_poisson_workspace_bytes": (_sz, [_vp]),
@@ -51,9 +51,8 @@ SYMBOLS = {
 
 
 def _load():
-    path = _build.LIB
-    if not os.path.exists(path):
-        path = _build.build()          # compiling the product is not a fallback; failure raises
+    path = _build.build()              # returns at once when the library is newer than its sources; compiling the
+                                       # product is not a fallback, and a failed build raises
     lib = C.CDLL(path)
     for name, (res, args) in SYMBOLS.items():
         f = getattr(lib, name)         # AttributeError if the library does not export it
@@ -128,6 +127,11 @@ def dks_poisson_solve_host(plan, rho_host, phi_host, stream=None):
 def dks_poisson_solve_host_async(plan, rho_host, phi_host, stream=None):
     return _check(lib.dks_poisson_solve_host_async(plan, _ptr(rho_host), _ptr(phi_host), stream),
                   "dks_poisson_solve_host_async")
+
+
+def dks_poisson_step_host_async(plan, hx, hy, hz, rho_host, phi_host, stream=None):
+    return _check(lib.dks_poisson_step_host_async(plan, float(hx), float(hy), float(hz), _ptr(rho_host), _ptr(phi_host), stream),
+                  "dks_poisson_step_host_async")
 
 
 def dks_poisson_host_sync(plan):
@@ -265,6 +269,14 @@ class PoissonPlan:
         import torch
 
         dks_poisson_solve_host_async(self._plan, rho_host, phi_host, torch.cuda.current_stream().cuda_stream)
+        return phi_host
+
+    def step_host_async(self, h, rho_host, phi_host):
+        """One time step with new spacings h: Green's rebuild overlapped with the copy of rho; finish with host_sync()."""
+        import torch
+
+        self.h = tuple(float(v) for v in h)
+        dks_poisson_step_host_async(self._plan, *self.h, rho_host, phi_host, torch.cuda.current_stream().cuda_stream)
         return phi_host
 
     def host_sync(self):

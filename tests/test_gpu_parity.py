@@ -263,9 +263,8 @@ def test_repeated_solves_are_bit_identical(torch_cuda, dks, workloads, n):
         plan.close()
 
 
-def test_greens_hat_matches_oracle_transform(torch_cuda, dks, oracle):
-    # Ghat octant (scale folded in) against numpy's FFT of the oracle-independent definition is NOT
-    # used here; instead: solve of a unit point charge at the origin returns exactly G on the mesh.
+def test_greens_point_charge_at_origin_returns_G(torch_cuda, dks, oracle):
+    # solve of a unit point charge at the origin returns exactly G on the mesh (a0 through the whole pipeline)
     n, h = (16, 16, 16), (1e-3, 2e-3, 5e-4)
     rho = np.zeros((16, 16, 16))
     rho[0, 0, 0] = 1.0 / (h[0] * h[1] * h[2])
@@ -273,6 +272,149 @@ def test_greens_hat_matches_oracle_transform(torch_cuda, dks, oracle):
     for (i, j, k) in [(1, 0, 0), (0, 1, 0), (0, 0, 1), (3, 4, 5), (15, 15, 15)]:
         g = oracle.green(i * h[0], j * h[1], k * h[2])
         assert abs(got[k, j, i] - g) <= 1e-11 * np.max(np.abs(got))
+
+
+# ---- step a0 directly: the Green's octant of dks_greens_setup against the oracle's FT{Gt} ----
+@pytest.mark.parametrize("n,h,g0", [((16, 8, 32), (1e-3, 2e-3, 5e-4), None),           # generic x, y; r16 z
+                                     ((32, 64, 16), (2e-4, 3e-4, 1e-4), 7.5e12),         # r16 x, y; generic z
+                                     ((128, 32, 64), (1e-4, 2e-4, 4e-4), None),
+                                     ((256, 16, 8), (1e-4, 1e-3, 1e-3), None),
+                                     ((8, 8, 8), (1e-3, 1e-3, 1e-3), None)])
+def test_greens_octant_matches_oracle(torch_cuda, dks, oracle, n, h, g0):
+    nx, ny, nz = n
+    plan = dks.PoissonPlan(n, h, g0=g0)
+    try:
+        got = plan.greens_hat()                              # scale hx hy hz / (8 nx ny nz) folded in
+    finally:
+        plan.close()
+    op = oracle.Plan(n, h, g0=g0, precision="ld")
+    try:
+        ref = op.ghat_octant() * (h[0] * h[1] * h[2] / (8.0 * nx * ny * nz))
+    finally:
+        op.close()
+    assert got.shape == ref.shape == (nz + 1, ny + 1, nx + 1)
+    # Ghat is a sum of 8 nx ny nz terms of mixed sign: the bound is relative to its largest entry
+    assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(np.abs(ref))
+    assert np.linalg.norm((got - ref).ravel()) <= 1e-13 * np.linalg.norm(ref.ravel())
+
+
+def test_greens_octant_pad_columns_stay_negligible(torch_cuda, dks):
+    # The pad entries nx < kx < gpitch of every octant row are the imaginary partners of valid columns in the packed
+    # y / z transforms of the setup (dks_greens_r16.cuh): they start at zero and may only pick up the rounding leakage of
+    # their partner column; a NaN or a large value there would contaminate column nx.  Read them raw from the workspace.
+    torch = torch_cuda
+    for n in [(32, 16, 64), (16, 32, 8), (64, 64, 64)]:
+        nx, ny, nz = n
+        h_ = dks.dks_poisson_plan_create(*n, 1e-3, 2e-3, 5e-4)
+        try:
+            nbytes = dks.dks_poisson_workspace_bytes(h_)
+            ws = torch.full((nbytes // 8,), float("nan"), dtype=torch.float64, device="cuda")
+            dks.dks_poisson_set_workspace(h_, ws, nbytes)
+            dks.dks_greens_setup(h_)
+            torch.cuda.synchronize()
+            gpitch = (nx + 1 + 7) // 8 * 8
+            off = ((16 * nx * ny * (nz + 1) + 255) // 256 * 256) // 8        # the octant follows buffer A
+            G = ws[off: off + gpitch * (ny + 1) * (nz + 1)].view(nz + 1, ny + 1, gpitch)
+            assert torch.all(torch.isfinite(G))
+            scale = 1e-3 * 2e-3 * 5e-4 / (8.0 * nx * ny * nz)   # folded into the valid entries by the last axis pass only
+            assert float(G[:, :, nx + 1:].abs().max()) <= 1e-14 * float(G[:, :, : nx + 1].abs().max()) / scale
+            assert torch.all(G[:, :, nx + 2:] == 0.0)        # only column nx + 1 has a valid partner (column nx)
+        finally:
+            dks.dks_poisson_plan_destroy(h_)
+
+
+# ---- f1: the per-step sequence of PAPER.md:132 (h changes every step) ------------------------------------
+def test_step_host_async_rebuilds_every_step(torch_cuda, dks, oracle, workloads):
+    torch = torch_cuda
+    n = (32, 16, 64)
+    hs = [(2e-4 * (1 + 0.1 * i), 3e-4 * (1 - 0.05 * i), 1e-4 * (1 + 0.2 * i)) for i in range(5)]
+    rhos = [workloads.random_rho(n, seed=90 + i) for i in range(5)]
+    plan = dks.PoissonPlan(n, hs[0])
+    try:
+        h_in = [torch.from_numpy(r).pin_memory() for r in rhos]
+        h_out = [torch.empty_like(t).pin_memory() for t in h_in]
+        for h, a, b in zip(hs, h_in, h_out):
+            plan.step_host_async(h, a, b)
+        plan.host_sync()
+        for h, r, b in zip(hs, rhos, h_out):
+            check(b.numpy(), oracle.solve(r, n, h, precision="ld"))
+    finally:
+        plan.close()
+
+
+def test_rebuild_on_side_stream_between_pipelined_solves(torch_cuda, dks, oracle, workloads):
+    # dks_greens_setup on its own stream between solve_host_async calls: the rebuild must wait for the previous P3
+    torch = torch_cuda
+    n = (64, 32, 32)
+    hs = [(1e-4 * (1 + i), 2e-4, 3e-4 / (1 + i)) for i in range(4)]
+    rhos = [workloads.random_rho(n, seed=60 + i) for i in range(4)]
+    side = torch.cuda.Stream()
+    plan = dks.PoissonPlan(n, hs[0])
+    try:
+        dks.dks_poisson_set_stream(plan.handle, side.cuda_stream)
+        h_in = [torch.from_numpy(r).pin_memory() for r in rhos]
+        h_out = [torch.empty_like(t).pin_memory() for t in h_in]
+        for h, a, b in zip(hs, h_in, h_out):
+            dks.dks_poisson_set_spacing(plan.handle, *h)
+            dks.dks_greens_setup(plan.handle)
+            plan.solve_host_async(a, b)
+        plan.host_sync()
+        for h, r, b in zip(hs, rhos, h_out):
+            check(b.numpy(), oracle.solve(r, n, h, precision="ld"))
+    finally:
+        torch.cuda.synchronize()
+        plan.close()
+
+
+def test_two_live_plans_of_different_shapes(torch_cuda, dks, oracle, workloads):
+    # the kernels' shared-memory attributes are process-wide: a small plan must not lower what a large one needs
+    torch = torch_cuda
+    big, small = ((8, 8, 512), (1e-3, 1e-3, 5e-5)), ((16, 16, 16), (1e-3, 1e-3, 1e-3))
+    rb, rs = workloads.random_rho(big[0], seed=1), workloads.random_rho(small[0], seed=2)
+    pb = dks.PoissonPlan(*big)
+    ps = dks.PoissonPlan(*small)
+    try:
+        db, ds = torch.from_numpy(rb).cuda(), torch.from_numpy(rs).cuda()
+        for _ in range(2):
+            check(pb.solve(db).cpu().numpy(), oracle.solve(rb, *big, precision="ld"))
+            check(ps.solve(ds).cpu().numpy(), oracle.solve(rs, *small, precision="ld"))
+            pb.set_spacing(big[1])
+            ps.set_spacing(small[1])
+    finally:
+        pb.close()
+        ps.close()
+
+
+# ---- refusals ---------------------------------------------------------------------------------------------------------
+def test_refusals(torch_cuda, dks, workloads):
+    torch = torch_cuda
+    n, h = (16, 16, 16), (1e-3, 1e-3, 1e-3)
+    d = torch.zeros(16 * 16 * 16 + 1, dtype=torch.float64, device="cuda")
+    plan = dks.PoissonPlan(n, h, slab_planes=5)
+    try:
+        with pytest.raises(dks.DksError) as e:               # rho not 16-byte aligned
+            dks.dks_poisson_solve(plan.handle, d.data_ptr() + 8, d.data_ptr(), None)
+        assert e.value.status == dks.DKS_ERR_INVALID_ARG and "aligned" in str(e.value)
+        with pytest.raises(dks.DksError) as e:               # batched solve on a slabbed plan
+            dks.dks_poisson_solve_batch(plan.handle, d, d, 2, None)
+        assert e.value.status == dks.DKS_ERR_INVALID_ARG
+        with pytest.raises(dks.DksError) as e:               # the attached workspace cannot hold a batch of 4
+            dks.dks_poisson_set_max_batch(plan.handle, 4)
+        assert e.value.status == dks.DKS_ERR_WORKSPACE_TOO_SMALL
+        with pytest.raises(dks.DksError) as e:               # nor the unslabbed B
+            dks.dks_poisson_set_slab_planes(plan.handle, 17)
+        assert e.value.status == dks.DKS_ERR_WORKSPACE_TOO_SMALL
+        plan.solve(d[:4096].view(16, 16, 16))                # the plan still works after the refusals
+        torch.cuda.synchronize()
+    finally:
+        plan.close()
+    big = dks.dks_poisson_plan_create(8, 8, 1024, 1e-3, 1e-3, 1e-3)
+    try:
+        with pytest.raises(dks.DksError) as e:               # (nz + 1) * nbatch exceeds the grid limit of the y passes
+            dks.dks_poisson_set_max_batch(big, 64)
+        assert e.value.status == dks.DKS_ERR_INVALID_ARG and "65535" in str(e.value)
+    finally:
+        dks.dks_poisson_plan_destroy(big)
 
 
 def test_solve_host_path(torch_cuda, dks, oracle, workloads):
