@@ -41,7 +41,10 @@ def parse():
     ap.add_argument("--slab", type=int, default=None, help="planes per P2-P4 slab (default: the plan's automatic choice)")
     ap.add_argument("--prof-steps", type=int, default=50, help="extra solves with per-launch events, for the per-pass split")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--ref-full", action="store_true", help="--impl reference: time full-size oracle solves")
+    ap.add_argument("--ref-sample", action="store_true",
+                    help="--impl reference: time the central half-extent sub-mesh instead of the full mesh (reported unscaled, under its own workload name)")
+    ap.add_argument("--repeats", type=int, default=5, help="timed windows of --steps solves each; the median is reported")
+    ap.add_argument("--sustained-s", type=float, default=2.0, help="length of the additional back-to-back run (0 = skip)")
     return ap.parse_args()
 
 
@@ -76,42 +79,55 @@ def whole_job_value(world: int, steps: int, ms_max: float) -> float:
 
 
 class ClockSampler:
-    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+    """One long-running `nvidia-smi -lms 20` whose rows are stamped on arrival; summary(t0, t1) looks at the rows that
+    arrived inside a window of host time (time.perf_counter()).  Windows shorter than the period see few or no rows:
+    `samples` says how many, and the summary then falls back to the rows nearest to the window."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    PERIOD_MS = 20
 
     def __init__(self, index=0):
-        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+        self.index, self.rows, self._t, self._p = index, [], None, None
 
     def _run(self):
-        while not self._stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                self.rows.append([c.strip() for c in out.strip().split(",")])
-            except Exception:
-                pass
-            self._stop.wait(0.1)
+        for line in self._p.stdout:
+            self.rows.append((time.perf_counter(), [c.strip() for c in line.strip().split(",")]))
 
     def __enter__(self):
-        self._t = threading.Thread(target=self._run, daemon=True)
-        self._t.start()
+        try:
+            self._p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                        "-i", str(self.index), "-lms", str(self.PERIOD_MS)],
+                                       stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        except Exception:
+            self._p = None
         return self
 
     def __exit__(self, *a):
-        self._stop.set()
-        self._t.join(timeout=10)
+        if self._p is not None:
+            self._p.terminate()
+            try:
+                self._p.wait(timeout=5)
+            except Exception:
+                self._p.kill()
+            self._t.join(timeout=5)
 
-    def summary(self):
-        sm, mx, reasons = [], [], set()
+    def summary(self, t0=None, t1=None):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        rows = [r for (t, r) in self.rows if (t0 is None or t >= t0) and (t1 is None or t <= t1)]
+        inside = len(rows)
+        if not rows and self.rows and t0 is not None:      # window shorter than the sampling period: nearest rows
+            mid = 0.5 * (t0 + (t1 if t1 is not None else t0))
+            rows = [r for (_, r) in sorted(self.rows, key=lambda tr: abs(tr[0] - mid))[:2]]
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in rows:
             if len(r) < 7:
                 continue
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
             except ValueError:
                 continue
             for name, v in zip(names, r[3:7]):
@@ -120,78 +136,71 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "reasons": sorted(reasons), "samples": inside, "period_ms": self.PERIOD_MS}
 
 
 # ------------------------------------------------------------------------------------------------
 # CPU oracle legs (the only places bench.py executes oracle/)
 # ------------------------------------------------------------------------------------------------
-def _work(n):
-    import math
-    N = 8.0 * n[0] * n[1] * n[2]
-    return N * math.log2(N)
-
-
-def oracle_full_solve(w, rho, repeats=1):
-    """Times `repeats` full oracle solves (double build, FT{G} precomputed as for the GPU timer)."""
+def oracle_full_solve(w, rho, budget_s=20.0):
+    """One untimed full oracle solve (first touch of its 2 x 2 GB work arrays at 256^3), then timed full solves until
+    about `budget_s` of CPU time is spent, at least one (double build, FT{G} precomputed as for the GPU timer)."""
     from oracle import oracle as O
     plan = O.Plan(w.n, w.h, precision="d")
     try:
         t0 = time.perf_counter()
-        for _ in range(repeats):
+        plan.solve(rho)
+        first = time.perf_counter() - t0
+        reps = max(1, min(20, int((budget_s - first) / max(first, 1e-3))))
+        t0 = time.perf_counter()
+        for _ in range(reps):
             plan.solve(rho)
-        dt = (time.perf_counter() - t0) / repeats
+        dt = (time.perf_counter() - t0) / reps
     finally:
         plan.close()
-    return dt, O.num_threads("d")
-
-
-def oracle_sample_plan(w, rho):
-    """Bounded sample of the workload: the central half-extent sub-mesh (1/8 of the nodes) of the same
-    rho, same spacings.  Returns (plan, sub_rho, n_sub)."""
-    from oracle import oracle as O
-    import numpy as np
-    nx, ny, nz = w.n
-    sx, sy, sz = max(nx // 2, 8), max(ny // 2, 8), max(nz // 2, 8)
-    x0, y0, z0 = (nx - sx) // 2, (ny - sy) // 2, (nz - sz) // 2
-    sub = np.ascontiguousarray(rho[z0:z0 + sz, y0:y0 + sy, x0:x0 + sx])
-    return O.Plan((sx, sy, sz), w.h, precision="d"), sub, (sx, sy, sz)
+    return dt, reps, first, O.num_threads("d")
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, on the host cores, rank 0 only."""
+    """--impl reference: the CPU oracle as it stands, on the host cores, rank 0 only.  Every step is one FULL oracle
+    solve of the benchmarked mesh (2-3 s at 256^3), ms_per_step the wall time a step took.  --ref-sample times the
+    central half-extent sub-mesh instead and says so in config.workload; nothing is extrapolated."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from paper_1509_07685_b200 import workloads as W
     from oracle import oracle as O
+    import numpy as np
     w = W.config(args.config)
     rho = W.make_rho(w)
-    if args.ref_full:
-        plan, sub, n_sub, scale = O.Plan(w.n, w.h, precision="d"), rho, w.n, 1.0
-        sample = f"each step = one full oracle solve of {w.name} (double build, FT{{G}} precomputed)"
-    else:
-        plan, sub, n_sub = oracle_sample_plan(w, rho)
-        scale = _work(n_sub) / _work(w.n)
-        sample = (f"each step = one oracle solve (double build, FT{{G}} precomputed) of the central "
-                  f"{n_sub[0]}x{n_sub[1]}x{n_sub[2]} sub-mesh of {w.name}; solves/s scaled by the N*log2(N) "
-                  f"work ratio {scale:.4f} (N = padded points)")
+    name = workload_name(w)
+    n = w.n
+    sample = f"each step = one full oracle solve of {w.name} (double build, OpenMP, FT{{G}} precomputed and not timed)"
+    if args.ref_sample:
+        nx, ny, nz = w.n
+        n = (max(nx // 2, 8), max(ny // 2, 8), max(nz // 2, 8))
+        x0, y0, z0 = (nx - n[0]) // 2, (ny - n[1]) // 2, (nz - n[2]) // 2
+        rho = np.ascontiguousarray(rho[z0:z0 + n[2], y0:y0 + n[1], x0:x0 + n[0]])
+        name = f"central {n[0]}x{n[1]}x{n[2]} sub-mesh of {name} (NOT the benchmarked mesh; --ref-sample)"
+        sample = f"each step = one oracle solve of the central {n[0]}x{n[1]}x{n[2]} sub-mesh of {w.name} (double build, FT{{G}} precomputed)"
+    plan = O.Plan(n, w.h, precision="d")
     try:
         for _ in range(args.warmup):
-            plan.solve(sub)
+            plan.solve(rho)
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            plan.solve(sub)
+            plan.solve(rho)
         dt = time.perf_counter() - t0
     finally:
         plan.close()
-    value = args.steps / dt * scale
+    value = args.steps / dt
     cores = O.num_threads("d")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / value, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(w), "timing": "host wall clock around the oracle's solve"},
+        "config": {"workload": name, "timing": "host wall clock around the oracle's solves"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -235,21 +244,40 @@ def run_ours(args):
     for _ in range(args.warmup):
         plan.solve(d_rho, d_phi)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    windows, sustained = [], None
     with ClockSampler(local) as clocks:
-        e0.record(stream)
-        for _ in range(args.steps):
-            plan.solve(d_rho, d_phi)
-        e1.record(stream)
         barrier()
-    ms_total = e0.elapsed_time(e1)
+        t_first = time.perf_counter()
+        for _ in range(max(1, args.repeats)):            # each window: exactly --steps solves between two events
+            barrier()
+            e0.record(stream)
+            for _ in range(args.steps):
+                plan.solve(d_rho, d_phi)
+            e1.record(stream)
+            barrier()
+            windows.append(max_over_ranks(e0.elapsed_time(e1), "cuda"))
+        t_last = time.perf_counter()
+        clocks_timed = clocks.summary(t_first, t_last)
+        if args.sustained_s > 0:                         # a per-time-step solver runs for minutes: the same loop for >= 2 s
+            n_sus = max(args.steps, int(args.sustained_s * 1e3 / (sorted(windows)[len(windows) // 2] / args.steps)) + 1)
+            barrier()
+            ts0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(n_sus):
+                plan.solve(d_rho, d_phi)
+            e1.record(stream)
+            barrier()
+            ts1 = time.perf_counter()
+            ms_sus = max_over_ranks(e0.elapsed_time(e1), "cuda")
+            sustained = {"steps": n_sus, "ms_per_step": ms_sus / n_sus, "value": whole_job_value(world, n_sus, ms_sus),
+                         "unit": UNIT, "clocks": clocks.summary(ts0 + 0.5 * (ts1 - ts0), ts1)}   # clocks of the second half
+    ms_total = sorted(windows)[len(windows) // 2]        # median window
     # per-pass split: a second, untimed-for-the-headline run with events around every launch
     dks.dks_poisson_set_profiling(plan.handle, min(args.prof_steps, 256))
     for _ in range(min(args.prof_steps, 256)):
         plan.solve(d_rho, d_phi)
     pass_ms = dks.dks_poisson_pass_times(plan.handle)
     dks.dks_poisson_set_profiling(plan.handle, 0)
-    ms_total = max_over_ranks(ms_total, "cuda")
     ms_per_step = ms_total / args.steps
     value = whole_job_value(world, args.steps, ms_total)
 
@@ -309,6 +337,41 @@ def run_ours(args):
     e2e_ms = (time.perf_counter() - t0) * 1e3
     e2e_value = whole_job_value(world, args.e2e_steps, max_over_ranks(e2e_ms, "cuda"))
     e2e_sync_value = whole_job_value(world, args.e2e_steps, max_over_ranks(e2e_sync_ms, "cuda"))
+    # the step the paper runs: new spacings every step, Green's rebuild beside the rho copy
+    for i in range(3):
+        plan.step_host_async(w.h, h_rho, outs[i & 1])
+    plan.host_sync()
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.e2e_steps):
+        hh = tuple(v * (1.0 + 1e-3 * (i + 1)) for v in w.h)
+        plan.step_host_async(hh, h_rho, outs[i & 1])
+    plan.host_sync()
+    barrier()
+    e2e_rebuild_value = whole_job_value(world, args.e2e_steps, max_over_ranks((time.perf_counter() - t0) * 1e3, "cuda"))
+    plan.set_spacing(w.h)
+    # yardstick: what the host link gives for the same buffers (pinned, one mesh per copy), one direction at a time
+    # and both at once on two streams -- the pipelined e2e cannot beat the bidirectional figure
+    s_a, s_b = torch.cuda.Stream(), torch.cuda.Stream()
+    d_tmp = torch.empty_like(d_rho)
+
+    def _copy_rate(h2d, d2h, reps=5):
+        torch.cuda.synchronize()
+        t = time.perf_counter()
+        for _ in range(reps):
+            if h2d:
+                with torch.cuda.stream(s_a):
+                    d_tmp.copy_(h_rho, non_blocking=True)
+            if d2h:
+                with torch.cuda.stream(s_b):
+                    h_phi2.copy_(d_phi, non_blocking=True)
+        torch.cuda.synchronize()
+        return reps * nbytes / (time.perf_counter() - t) / 1e9
+
+    link = {"h2d_gbs": _copy_rate(True, False), "d2h_gbs": _copy_rate(False, True),
+            "bidirectional_gbs_per_direction": _copy_rate(True, True)}
+    link["steps_per_s_at_link_limit"] = link["bidirectional_gbs_per_direction"] * 1e9 / nbytes
+    del d_tmp
 
     if rank != 0:
         plan.close()
@@ -346,10 +409,10 @@ def run_ours(args):
     # ---- CPU oracle timed beside it (rank 0, N = 1 only) ---------------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        dt, cores = oracle_full_solve(w, rho)
+        dt, reps, first, cores = oracle_full_solve(w, rho)
         cpu = {"value": 1.0 / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"1 full solve of {w.name} by oracle/poisson_oracle.c (double build, OpenMP, "
-                         f"FT{{G}} precomputed and not timed), {dt:.2f} s"}
+               "sample": f"{reps} full solves of {w.name} by oracle/poisson_oracle.c (double build, OpenMP, FT{{G}} precomputed "
+                         f"and not timed) after one untimed solve ({first:.2f} s, first touch): {dt:.2f} s each"}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -361,12 +424,19 @@ def run_ours(args):
                           "working set fits the 126 MB L2 (L2-resident workload); no flush"),
                    "greens_setup": "precomputed, outside the timed region (DESIGN.md reading A11)",
                    "greens_setup_ms": greens_ms, "batched": batched},
-        "clocks": clocks.summary(),
+        "clocks": clocks_timed,
+        "timing": {"windows": len(windows), "ms_per_step_each": [t / args.steps for t in windows],
+                   "reported": "median window", "clock_sampling": f"nvidia-smi -lms {ClockSampler.PERIOD_MS} over all windows"},
+        "sustained": sustained,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                 "steps": args.e2e_steps, "timing": "host clock around the loop, device idle before and after",
                 "api": "dks_poisson_solve_host_async per step + one dks_poisson_host_sync (pinned host rho -> H2D -> P1..P5 -> "
                        "D2H -> host phi every step; copies of neighbouring steps overlap the solve)",
-                "blocking_api_value": e2e_sync_value},
+                "blocking_api_value": e2e_sync_value,
+                "with_greens_rebuild_per_step": {"value": e2e_rebuild_value, "unit": UNIT,
+                                                 "api": "dks_poisson_step_host_async (new spacings every step: Green's rebuild on its own "
+                                                        "stream beside the rho copy, PAPER.md:132) + one dks_poisson_host_sync"},
+                "host_link": link},
         "gpu_launches": launches * args.steps,
         "roofline": roofline,
     }
