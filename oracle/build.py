@@ -3,7 +3,8 @@
     python -m oracle.build
 
 produces oracle/liboracle_ld.so (REAL = long double: parity reference values) and
-oracle/liboracle_d.so (REAL = double: the timed CPU baseline) from oracle/poisson_oracle.c.
+oracle/liboracle_d.so (REAL = double: the timed CPU baseline) from oracle/poisson_oracle.c and oracle/field_ops_oracle.c.
+ORACLE_SANITIZE=1 adds -fsanitize=address,undefined (used by the sanitizer run recorded under profiles/).
 """
 from __future__ import annotations
 
@@ -12,12 +13,12 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "poisson_oracle.c")
+SRCS = [os.path.join(HERE, "poisson_oracle.c"), os.path.join(HERE, "field_ops_oracle.c")]
 LIBS = {"ld": os.path.join(HERE, "liboracle_ld.so"), "d": os.path.join(HERE, "liboracle_d.so")}
 
 
 def _stale(lib: str) -> bool:
-    return (not os.path.exists(lib)) or os.path.getmtime(lib) < os.path.getmtime(SRC)
+    return (not os.path.exists(lib)) or any(os.path.getmtime(lib) < os.path.getmtime(src) for src in SRCS)
 
 
 def build(force: bool = False) -> dict:
@@ -26,9 +27,11 @@ def build(force: bool = False) -> dict:
             continue
         # -ffp-contract=off / no -ffast-math: IEEE arithmetic exactly as written.
         cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-               "-Wall", "-Wextra", SRC, "-o", lib, "-lm"]
+               "-Wall", "-Wextra"] + SRCS + ["-o", lib, "-lm"]
         if kind == "ld":
             cmd.insert(1, "-DORACLE_LD")
+        if os.environ.get("ORACLE_SANITIZE") == "1":
+            cmd[1:1] = ["-fsanitize=address,undefined", "-fno-omit-frame-pointer", "-g"]
         subprocess.run(cmd, check=True)
     return LIBS
 

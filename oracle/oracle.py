@@ -42,6 +42,11 @@ def _lib(precision: str):
         f.argtypes = [C.c_int] * 3 + [C.c_double] * 4 + [dp, C.POINTER(C.c_longlong), C.c_int, dp]
         f.restype = None
         f = getattr(lib, p + "num_threads"); f.argtypes = []; f.restype = C.c_int
+        f = getattr(lib, p + "cic_deposit")
+        f.argtypes = [C.c_int] * 3 + [C.c_double] * 6 + [dp, dp, dp, dp, C.c_longlong, dp]; f.restype = C.c_longlong
+        f = getattr(lib, p + "gradient"); f.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [dp, dp, dp, dp]; f.restype = None
+        f = getattr(lib, p + "cic_gather")
+        f.argtypes = [C.c_int] * 3 + [C.c_double] * 6 + [dp, dp, dp, dp, C.c_longlong, dp]; f.restype = None
         _libs[precision] = (lib, p)
     return _libs[precision]
 
@@ -148,3 +153,35 @@ def direct_sum(rho, n, h, g0=None, precision="ld"):
 def num_threads(precision="d") -> int:
     lib, p = _lib(precision)
     return getattr(lib, p + "num_threads")()
+
+
+# ---- the steps adjacent to the solve (oracle/field_ops_oracle.c; readings F1-F4) --------------------------------------
+def cic_deposit(n, h, origin, x, y, z, q, precision="ld"):
+    """rho [nz][ny][nx] from particles at physical positions (x, y, z) with charges q; returns (rho, particles kept)."""
+    lib, p = _lib(precision)
+    nx, ny, nz = n
+    x, y, z, q = (np.ascontiguousarray(a, dtype=np.float64) for a in (x, y, z, q))
+    rho = np.empty((nz, ny, nx), dtype=np.float64)
+    kept = getattr(lib, p + "cic_deposit")(nx, ny, nz, *h, *origin, _dp(x), _dp(y), _dp(z), _dp(q), len(x), _dp(rho))
+    return rho, int(kept)
+
+
+def gradient(phi, n, h, precision="ld"):
+    """(Ex, Ey, Ez) = -grad(phi), second-order differences (F3)."""
+    lib, p = _lib(precision)
+    nx, ny, nz = n
+    phi = np.ascontiguousarray(phi, dtype=np.float64)
+    ex, ey, ez = (np.empty_like(phi) for _ in range(3))
+    getattr(lib, p + "gradient")(nx, ny, nz, *h, _dp(phi), _dp(ex), _dp(ey), _dp(ez))
+    return ex, ey, ez
+
+
+def cic_gather(field, n, h, origin, x, y, z, precision="ld"):
+    """Trilinear interpolation of a node field to the particles (F4); 0 for dropped particles."""
+    lib, p = _lib(precision)
+    nx, ny, nz = n
+    field = np.ascontiguousarray(field, dtype=np.float64)
+    x, y, z = (np.ascontiguousarray(a, dtype=np.float64) for a in (x, y, z))
+    out = np.empty(len(x), dtype=np.float64)
+    getattr(lib, p + "cic_gather")(nx, ny, nz, *h, *origin, _dp(field), _dp(x), _dp(y), _dp(z), len(x), _dp(out))
+    return out

@@ -117,6 +117,21 @@ def cic_deposit(pos: np.ndarray, q: float, n, h) -> np.ndarray:
     return rho.reshape(nz, ny, nx)
 
 
+def particles(w: Workload, origin=None, count=None):
+    """The config's particles as physical coordinates x, y, z [m] (node (i, j, k) sits at origin + (i hx, j hy, k hz);
+    default origin: the mesh centred on 0) and charges q [C]: four float64 arrays.  `count` keeps the first particles only."""
+    pos, q = _positions_and_charge(w)
+    if count is not None:
+        pos = pos[:count]
+    h = np.array(w.h, dtype=np.float64)
+    if origin is None:
+        origin = -0.5 * (np.array(w.n, dtype=np.float64) - 1.0) * h
+    origin = np.asarray(origin, dtype=np.float64)
+    xyz = origin + pos * h
+    return (np.ascontiguousarray(xyz[:, 0]), np.ascontiguousarray(xyz[:, 1]), np.ascontiguousarray(xyz[:, 2]),
+            np.full(len(pos), q, dtype=np.float64), tuple(float(v) for v in origin))
+
+
 def make_rho(w: Workload) -> np.ndarray:
     """The config's charge density, contiguous float64 [nz][ny][nx]."""
     pos, q = _positions_and_charge(w)
