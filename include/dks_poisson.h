@@ -166,6 +166,29 @@ const char *dks_poisson_pass_name(const dks_poisson_plan *plan, int pass); /* ke
  * (nx+1)(ny+1)(nz+1) doubles; synchronises.  For tests. */
 int dks_poisson_copy_greens_hat(dks_poisson_plan *plan, double *host_out);
 
+/* ---- The steps adjacent to the solve, on the device ------------------------------------------
+ * OPAL's particles come "with the respective interpolation operators" (IPPL); moving rho and
+ * phi between host and device costs "up to 55 %" of the run.  With the deposit before and the field evaluation after the
+ * solve on the device, only particle data (or nothing, if the particles live there) crosses the host link.  The paper
+ * gives no formulas; readings F1-F4: node (i,j,k) sits at origin + (i hx, j hy, k hz) with the plan's CURRENT
+ * spacings; cloud-in-cell (trilinear) weights; a particle is dropped unless 0 <= (X - ox)/hx < nx - 1 (likewise y, z);
+ * E = -grad(phi) by second-order differences (central inside, one-sided second order at the ends; every extent >= 8).
+ * All pointers are DEVICE pointers to contiguous fp64; meshes are [nz][ny][nx]; particle arrays hold np entries (SoA).
+ * Asynchronous on `stream`, no allocation, no synchronisation; none of them needs dks_greens_setup. */
+
+/* rho[node] = sum_p q_p w_p(node) / (hx hy hz) (C/m^3 for q in C).  rho is zeroed first (on `stream`).  The sums are
+ * fp64 atomics: order-free, so equal to a sequential sum only to a few ulp of each node's total. */
+int dks_deposit_cic(dks_poisson_plan *plan, const double *x_dev, const double *y_dev, const double *z_dev, const double *q_dev,
+                    long long np, double ox, double oy, double oz, double *rho_dev, void *stream);
+
+/* (ex, ey, ez) = -grad(phi) [V/m]; the outputs must not alias phi. */
+int dks_gradient(dks_poisson_plan *plan, const double *phi_dev, double *ex_dev, double *ey_dev, double *ez_dev, void *stream);
+
+/* Field at the particles: trilinear interpolation of (ex, ey, ez) with the deposit's weights; 0 for dropped particles. */
+int dks_gather_field(dks_poisson_plan *plan, const double *ex_dev, const double *ey_dev, const double *ez_dev,
+                     const double *x_dev, const double *y_dev, const double *z_dev, long long np, double ox, double oy, double oz,
+                     double *epx_dev, double *epy_dev, double *epz_dev, void *stream);
+
 /* Thread-local, NUL-terminated message describing the last failure in this thread ("" if none).  The library never
  * throws or aborts: every entry point reports through its status (the paper's DKS layer hands device errors back to
  * the host application in the same way). */

@@ -20,6 +20,7 @@
 #include "dks_passes_generic.cuh"
 #include "dks_passes_r16.cuh"
 #include "dks_greens_r16.cuh"
+#include "dks_field_ops.cuh"
 
 using namespace dks;
 
@@ -808,4 +809,66 @@ extern "C" int dks_poisson_solve_host(dks_poisson_plan *p, const double *rho_hos
     int rc = dks_poisson_solve_host_async(p, rho_host, phi_host, stream);
     if (rc) return rc;
     return dks_poisson_host_sync(p);
+}
+
+// ------------------------------------------------------------------------------------------------
+// f4: the steps adjacent to the solve (dks_field_ops.cuh)
+// ------------------------------------------------------------------------------------------------
+static ParticleFrame frame_of(const dks_poisson_plan *p, double ox, double oy, double oz)
+{
+    ParticleFrame f;
+    f.ox = ox; f.oy = oy; f.oz = oz; f.hx = p->hx; f.hy = p->hy; f.hz = p->hz;
+    return f;
+}
+
+static int particle_grid(const dks_poisson_plan *p, long long np)
+{
+    const long long blocks = (np + 255) / 256;
+    return (int)std::max<long long>(1, std::min<long long>(blocks, (long long)p->sm_count * 8 * 4));
+}
+
+extern "C" int dks_deposit_cic(dks_poisson_plan *p, const double *x, const double *y, const double *z, const double *q,
+                               long long np, double ox, double oy, double oz, double *rho, void *stream)
+{
+    if (!p || !rho || np < 0 || (np > 0 && (!x || !y || !z || !q))) return fail(DKS_ERR_INVALID_ARG, "plan, rho or a particle array is NULL, or np < 0");
+    if (!std::isfinite(ox) || !std::isfinite(oy) || !std::isfinite(oz)) return fail(DKS_ERR_INVALID_ARG, "origin must be finite");
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t nodes = (size_t)p->d.nx * p->d.ny * p->d.nz;
+    DKS_CUDA(cudaMemsetAsync(rho, 0, sizeof(double) * nodes, st));
+    if (np > 0)
+        cic_deposit_kernel<<<particle_grid(p, np), 256, 0, st>>>(x, y, z, q, np, frame_of(p, ox, oy, oz), p->d,
+                                                                  1.0 / (p->hx * p->hy * p->hz), rho);
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+extern "C" int dks_gradient(dks_poisson_plan *p, const double *phi, double *ex, double *ey, double *ez, void *stream)
+{
+    if (!p || !phi || !ex || !ey || !ez) return fail(DKS_ERR_INVALID_ARG, "plan or a field pointer is NULL");
+    if (phi == ex || phi == ey || phi == ez) return fail(DKS_ERR_INVALID_ARG, "the field components must not alias phi");
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    const MeshDims d = p->d;
+    gradient_kernel<<<dim3((d.nx + 127) / 128, d.ny, d.nz), 128, 0, static_cast<cudaStream_t>(stream)>>>(
+        phi, ex, ey, ez, d, 0.5 / p->hx, 0.5 / p->hy, 0.5 / p->hz);
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+extern "C" int dks_gather_field(dks_poisson_plan *p, const double *ex, const double *ey, const double *ez, const double *x,
+                                const double *y, const double *z, long long np, double ox, double oy, double oz,
+                                double *epx, double *epy, double *epz, void *stream)
+{
+    if (!p || !ex || !ey || !ez || np < 0 || (np > 0 && (!x || !y || !z || !epx || !epy || !epz)))
+        return fail(DKS_ERR_INVALID_ARG, "plan, a field or a particle array is NULL, or np < 0");
+    if (!std::isfinite(ox) || !std::isfinite(oy) || !std::isfinite(oz)) return fail(DKS_ERR_INVALID_ARG, "origin must be finite");
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    if (np > 0)
+        gather_field_kernel<<<particle_grid(p, np), 256, 0, static_cast<cudaStream_t>(stream)>>>(ex, ey, ez, x, y, z, np,
+                                                                                                  frame_of(p, ox, oy, oz), p->d, epx, epy, epz);
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
 }

@@ -46,6 +46,9 @@ SYMBOLS = {
     "dks_poisson_model_bytes": (_d, [_vp, _i]),
     "dks_poisson_pass_name": (C.c_char_p, [_vp, _i]),
     "dks_poisson_copy_greens_hat": (_i, [_vp, _vp]),
+    "dks_deposit_cic": (_i, [_vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp]),
+    "dks_gradient": (_i, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "dks_gather_field": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "dks_last_error": (C.c_char_p, []),
 }
 
@@ -194,6 +197,20 @@ def dks_poisson_copy_greens_hat(plan, host_out):
     return _check(lib.dks_poisson_copy_greens_hat(plan, _ptr(host_out)), "dks_poisson_copy_greens_hat")
 
 
+def dks_deposit_cic(plan, x, y, z, q, np_, origin, rho, stream=None):
+    return _check(lib.dks_deposit_cic(plan, _ptr(x), _ptr(y), _ptr(z), _ptr(q), int(np_), *(float(v) for v in origin),
+                                      _ptr(rho), stream), "dks_deposit_cic")
+
+
+def dks_gradient(plan, phi, ex, ey, ez, stream=None):
+    return _check(lib.dks_gradient(plan, _ptr(phi), _ptr(ex), _ptr(ey), _ptr(ez), stream), "dks_gradient")
+
+
+def dks_gather_field(plan, ex, ey, ez, x, y, z, np_, origin, epx, epy, epz, stream=None):
+    return _check(lib.dks_gather_field(plan, _ptr(ex), _ptr(ey), _ptr(ez), _ptr(x), _ptr(y), _ptr(z), int(np_),
+                                       *(float(v) for v in origin), _ptr(epx), _ptr(epy), _ptr(epz), stream), "dks_gather_field")
+
+
 # ---- convenience wrapper (still marshalling only) ---------------------------------------------------
 class PoissonPlan:
     """Owns a dks_poisson_plan and a torch-allocated workspace on the current CUDA device."""
@@ -281,6 +298,30 @@ class PoissonPlan:
 
     def host_sync(self):
         dks_poisson_host_sync(self._plan)
+
+    def deposit(self, x, y, z, q, origin, rho=None):
+        """CUDA float64 particle arrays (SoA) -> rho [nz, ny, nx] on torch's current stream."""
+        import torch
+
+        nx, ny, nz = self.n
+        if rho is None:
+            rho = torch.empty((nz, ny, nx), dtype=torch.float64, device=x.device)
+        dks_deposit_cic(self._plan, x, y, z, q, x.numel(), origin, rho, torch.cuda.current_stream().cuda_stream)
+        return rho
+
+    def gradient(self, phi):
+        import torch
+
+        ex, ey, ez = torch.empty_like(phi), torch.empty_like(phi), torch.empty_like(phi)
+        dks_gradient(self._plan, phi, ex, ey, ez, torch.cuda.current_stream().cuda_stream)
+        return ex, ey, ez
+
+    def gather(self, ex, ey, ez, x, y, z, origin):
+        import torch
+
+        epx, epy, epz = torch.empty_like(x), torch.empty_like(x), torch.empty_like(x)
+        dks_gather_field(self._plan, ex, ey, ez, x, y, z, x.numel(), origin, epx, epy, epz, torch.cuda.current_stream().cuda_stream)
+        return epx, epy, epz
 
     def greens_hat(self):
         import numpy as np
