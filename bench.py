@@ -373,6 +373,44 @@ def run_ours(args):
     link["steps_per_s_at_link_limit"] = link["bidirectional_gbs_per_direction"] * 1e9 / nbytes
     del d_tmp
 
+    # ---- f4: the whole space-charge step with the particles resident on the device (deposit -> solve -> E -> gather):
+    # nothing but a scalar crosses the host link (PAPER.md:160 names that link as the limiter)
+    field_ops = None
+    if world == 1:
+        px, py, pz, pq, origin = W.particles(w)
+        dpx, dpy, dpz, dpq = (torch.from_numpy(a).cuda() for a in (px, py, pz, pq))
+        n_p = dpx.numel()
+        f_rho = torch.empty_like(d_rho)
+
+        def space_charge_step():
+            plan.deposit(dpx, dpy, dpz, dpq, origin, f_rho)
+            plan.solve(f_rho, d_phi)
+            ex, ey, ez = plan.gradient(d_phi)
+            return plan.gather(ex, ey, ez, dpx, dpy, dpz, origin)
+
+        def timed(fn, reps=10):
+            for _ in range(2):
+                fn()
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+
+        ex, ey, ez = plan.gradient(d_phi)
+        field_ops = {
+            "particles": n_p,
+            "deposit_ms": timed(lambda: plan.deposit(dpx, dpy, dpz, dpq, origin, f_rho)),
+            "gradient_ms": timed(lambda: plan.gradient(d_phi)),
+            "gather_ms": timed(lambda: plan.gather(ex, ey, ez, dpx, dpy, dpz, origin)),
+        }
+        step_ms = timed(space_charge_step)
+        field_ops["device_resident_step"] = {"ms_per_step": step_ms, "value": 1e3 / step_ms, "unit": "steps/s",
+                                             "api": "dks_deposit_cic + dks_poisson_solve + dks_gradient + dks_gather_field, "
+                                                    "particles and meshes resident on the device; no host traffic"}
+        del dpx, dpy, dpz, dpq, f_rho, ex, ey, ez
+
     if rank != 0:
         plan.close()
         if distributed:
@@ -428,6 +466,7 @@ def run_ours(args):
         "timing": {"windows": len(windows), "ms_per_step_each": [t / args.steps for t in windows],
                    "reported": "median window", "clock_sampling": f"nvidia-smi -lms {ClockSampler.PERIOD_MS} over all windows"},
         "sustained": sustained,
+        "field_ops": field_ops,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                 "steps": args.e2e_steps, "timing": "host clock around the loop, device idle before and after",
                 "api": "dks_poisson_solve_host_async per step + one dks_poisson_host_sync (pinned host rho -> H2D -> P1..P5 -> "

@@ -189,6 +189,29 @@ int dks_gather_field(dks_poisson_plan *plan, const double *ex_dev, const double 
                      const double *x_dev, const double *y_dev, const double *z_dev, long long np, double ox, double oy, double oz,
                      double *epx_dev, double *epy_dev, double *epz_dev, void *stream);
 
+/* ---- One solve sharded over several GPUs (SURVEY.md sections 8(e), 8(f3)) ------------------------------------------------
+ * The paper never splits a solve: several MPI ranks share ONE GPU through CUDA IPC.  This is the
+ * contrasting B200 design: rank r of g (g a power of two <= 8; nx, ny, nz in [32, 256]) owns the y rows
+ * [r ny/g, (r+1) ny/g) of rho and phi and the half-spectrum planes kz in [r nz/g, (r+1) nz/g) (the last rank also plane
+ * nz).  P1 runs on the y slab and stores every output row directly into the receive buffer of the rank that owns its
+ * plane; P2, P3, P4 run on the kz slab and P4 stores every row into the receive buffer of the rank that owns its y row;
+ * P5 runs on the y slab.  The receive buffers are device pointers the caller makes peer-accessible (NVLink P2P /
+ * symmetric memory; plain local pointers when several ranks are emulated on one device), so both exchanges -- two
+ * all-to-alls of buffer A, 2 x 269 MB at 256^3 -- are the epilogues of the producing kernels, not separate collectives.
+ * Between the phases the caller runs its own inter-rank barrier (e.g. an NCCL barrier on the same stream).
+ *
+ *   dks_poisson_set_shard     before the workspace is attached; changes dks_poisson_workspace_bytes()
+ *   dks_greens_setup          every rank builds the full Green's octant (it only reads its own planes)
+ *   dks_poisson_shard_buffers this rank's two receive buffers (inside its workspace), to be published to the peers
+ *   dks_poisson_set_peers     tables of all ranks' receive buffers as seen from this device (entry `rank` = its own)
+ *   dks_poisson_solve_shard   phase 1 (P1), barrier, phase 2 (P2-P4), barrier, phase 3 (P5); rho_loc / phi_loc are this
+ *                             rank's y slabs, [nz][ny/g][nx] contiguous fp64 (rho_loc for phase 1, phi_loc for phase 3)
+ * A sharded plan refuses dks_poisson_solve. */
+int dks_poisson_set_shard(dks_poisson_plan *plan, int rank, int nranks);
+int dks_poisson_shard_buffers(dks_poisson_plan *plan, void **recv_p1_dev, void **recv_p4_dev);
+int dks_poisson_set_peers(dks_poisson_plan *plan, void *const *recv_p1_of_rank, void *const *recv_p4_of_rank);
+int dks_poisson_solve_shard(dks_poisson_plan *plan, int phase, const double *rho_loc_dev, double *phi_loc_dev, void *stream);
+
 /* Thread-local, NUL-terminated message describing the last failure in this thread ("" if none).  The library never
  * throws or aborts: every entry point reports through its status (the paper's DKS layer hands device errors back to
  * the host application in the same way). */

@@ -22,6 +22,20 @@
 namespace dks {
 
 constexpr int kCols = 8;   // columns per CTA of the strided passes
+
+// Sharded solve: rho / phi are split into y slabs over the ranks, the
+// half-spectrum planes kz into kz slabs.  P1 (z lines, y-slab local) stores every output row straight into the buffer of
+// the rank that owns its kz plane, and P4 (y lines, kz-slab local) stores every output row into the buffer of the rank that
+// owns its y row: base[] holds device pointers that are peer-mapped over NVLink (or local, when ranks are emulated on one
+// device), so the exchange is part of the producing kernel's epilogue instead of a separate all-to-all.
+constexpr int kMaxRanks = 8;
+struct PeerTable {
+    cplx *base[kMaxRanks];   // the receive buffer of every rank
+    int nranks;              // 1: not sharded
+    int lsplit;              // log2 of the slab thickness (planes per rank for P1, y rows per rank for P4)
+    int first;               // P1: first global y row of this rank's slab;  P4: first global kz plane of this rank's slab
+    int pitch;               // P1: global ny (rows per plane in the receiver);  P4: y rows per rank (rows per plane in the receiver)
+};
 #ifndef DKS_R16_OCC
 #define DKS_R16_OCC 512
 #endif
@@ -102,10 +116,10 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
 // ---------------------------------------------------------------------------------------------
 // P4: inverse y, crop to ny.  grid (nx / 8, nz + 1)
 // ---------------------------------------------------------------------------------------------
-template <int A, bool PDL>
+template <int A, bool PDL, bool SHARD = false>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, int kz0,
-             const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
+             const cplx *__restrict__ tw1, const cplx *__restrict__ tw2, PeerTable T)
 {
     extern __shared__ cplx ex[];
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
@@ -123,8 +137,14 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
     cplx out[8];
     combine_parities<8>(v, p, out);
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
-        stg_stream(&Aout[((size_t)(kz0 + kz) * ny + a + A * (i + 8 * p)) * nx + x], out[i]);
+    for (int i = 0; i < 8; ++i) {
+        const int yrow = a + A * (i + 8 * p);
+        if (SHARD) {                                      // row y goes to the rank that owns it: [nz+1][ny / nranks][nx] there
+            const int o = yrow >> T.lsplit;
+            stg_stream(&T.base[o][((size_t)(T.first + kz) * T.pitch + (yrow - (o << T.lsplit))) * nx + x], out[i]);
+        } else
+            stg_stream(&Aout[((size_t)(kz0 + kz) * ny + yrow) * nx + x], out[i]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -155,10 +175,10 @@ __device__ __forceinline__ int p1_a_of(int p, int s, int w)
     return s ? A - w : w;
 }
 
-template <int A, bool PDL>
+template <int A, bool PDL, bool SHARD = false>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d, int nb,
-             const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
+             const cplx *__restrict__ tw1, const cplx *__restrict__ tw2, PeerTable T)
 {
     extern __shared__ cplx ex[];
     constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
@@ -187,7 +207,14 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     if (t < tiles) prefetch(t);
     for (; t < tiles; t += gridDim.x) {
         const int yy = t / xtiles, y = yy % ny;
-        cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx + (size_t)y * nx + (size_t)(t % xtiles) * 2 * kCols + 2 * c;
+        const size_t xoff = (size_t)(t % xtiles) * 2 * kCols + 2 * c;
+        cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx + (size_t)y * nx + xoff;
+        // sharded: row k goes to the rank that owns plane k (the last rank also owns plane n): [planes][ny global][nx] there
+        auto row = [&](int k) -> cplx * {
+            if (!SHARD) return Aout + (size_t)k * ny * nx;
+            const int o = min(k >> T.lsplit, T.nranks - 1);
+            return T.base[o] + ((size_t)(k - (o << T.lsplit)) * T.pitch + T.first + y) * nx + xoff;
+        };
         cp_async_wait_all();
         __syncthreads();                                  // stage complete; last tile's exchange reads done
         cplx v[16];
@@ -213,10 +240,10 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
             cplx cm = cmake(__shfl_sync(0xffffffffu, v[15 - r].x, partner), __shfl_sync(0xffffffffu, v[15 - r].y, partner));
             if (a0) cm = r == 0 ? v[0] : v[16 - r];
             const cplx ck = v[r];
-            stg_stream2(Aout + (size_t)(2 * (a + A * r) + p) * ny * nx, cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
+            stg_stream2(row(2 * (a + A * r) + p), cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
                         cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x)));
         }
-        if (a0) stg_stream2(Aout + (size_t)N * ny * nx, cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
+        if (a0) stg_stream2(row(N), cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
     }
 }
 

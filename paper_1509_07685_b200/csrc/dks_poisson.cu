@@ -82,6 +82,14 @@ struct dks_poisson_plan {
     int slab = 0;                       // planes per slab, 1..nz+1
     bool slab_user = false;             // set through dks_poisson_set_slab_planes
     struct Step { int pass, kz0, planes; };     // pass 1..5
+    // sharded solve (dks_poisson_set_shard): this plan is rank `rank` of `nranks`; it owns y rows [y0, y0 + ny_loc) of rho / phi
+    // and half-spectrum planes [kz0, kz0 + planes_loc).  A1 = receive buffer of P1's rows [planes_loc][ny][nx] (it replaces A),
+    // A2 = receive buffer of P4's rows [nz+1][ny_loc][nx].
+    int rank = 0, nranks = 1, ny_loc = 0, y0 = 0, kz0 = 0, planes_loc = 0;
+    cplx *A2 = nullptr;
+    size_t offA2 = 0;
+    PeerTable peers1 = PeerTable(), peers2 = PeerTable();
+    bool peers_set = false;
     int max_batch = 1;                  // meshes per dks_poisson_solve_batch call the workspace is sized for
     bool pdl = false;                   // programmatic dependent launch between the r16 passes (small meshes)
     std::vector<Step> steps;            // the launch list of one solve
@@ -136,10 +144,15 @@ static void compute_layout(dks_poisson_plan *p)
     const size_t nx = p->d.nx, ny = p->d.ny, nz = p->d.nz;
     size_t off = 0;
     const size_t nbm = (size_t)p->max_batch;
-    p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1) * nbm, 256);
+    if (p->nranks > 1) {                // A1 [planes_loc][ny][nx], A2 [nz+1][ny_loc][nx]
+        p->offA = off; off = align_up(off + 16 * nx * ny * (size_t)p->planes_loc, 256);
+        p->offA2 = off; off = align_up(off + 16 * nx * (size_t)p->ny_loc * (nz + 1), 256);
+    } else {
+        p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1) * nbm, 256);
+    }
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
     p->offS = off; off = align_up(off + 2 * align_up(8 * nx * ny * nz, 256), 256);
-    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)p->slab * nbm, 256);
+    p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)(p->nranks > 1 ? p->planes_loc : p->slab) * nbm, 256);
     p->need_bytes = off;
     p->steps.clear();
     p->steps.push_back({ 1, 0, 0 });
@@ -156,6 +169,8 @@ static void bind_workspace(dks_poisson_plan *p)
 {
     char *b = static_cast<char *>(p->ws);
     p->A = reinterpret_cast<cplx *>(b + p->offA);
+    p->A2 = p->nranks > 1 ? reinterpret_cast<cplx *>(b + p->offA2) : nullptr;
+    p->peers_set = false;
     p->B = reinterpret_cast<cplx *>(b + p->offB);
     p->G = reinterpret_cast<double *>(b + p->offG);
     p->stage = reinterpret_cast<double *>(b + p->offS);
@@ -278,6 +293,8 @@ static int r16_set_attributes()
 #define X(A_)                                                                                                         \
     DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
     DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16<A_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Geom<A_>::SMEM));  \
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
@@ -323,11 +340,11 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
     switch (s.pass) {
     case 1: {
         const int tiles = d.nx / (2 * kCols) * d.ny * nb, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
-        launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, nb, p->tw1[2], p->tw[2]);
+        launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, nb, p->tw1[2], p->tw[2], PeerTable());
         break;
     }
     case 2: launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
-    case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1], PeerTable()); break;
     case 5: launch_pdl(p->pdl, p5_z_c2r_r16<A, false>, p5_z_c2r_r16<A, true>, dim3(d.nx / (2 * kCols), d.ny, nb), dim3(T), S, st, p->A, phi, d, p->tw1[2], p->tw[2]); break;
     }
 }
@@ -671,6 +688,7 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
     if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
     if (nb < 1 || nb > p->max_batch)
         return fail(DKS_ERR_INVALID_ARG, "batch of %d meshes: the plan is sized for at most %d (dks_poisson_set_max_batch)", nb, p->max_batch);
+    if (p->nranks > 1) return fail(DKS_ERR_INVALID_ARG, "this plan is one rank of a sharded solve: use dks_poisson_solve_shard");
     if (nb > 1 && p->slab != p->d.nz + 1)
         return fail(DKS_ERR_INVALID_ARG, "batched solves need the default pipeline (no slabs)");
     if ((reinterpret_cast<uintptr_t>(rho) | reinterpret_cast<uintptr_t>(phi)) % 16)
@@ -869,6 +887,126 @@ extern "C" int dks_gather_field(dks_poisson_plan *p, const double *ex, const dou
     if (np > 0)
         gather_field_kernel<<<particle_grid(p, np), 256, 0, static_cast<cudaStream_t>(stream)>>>(ex, ey, ez, x, y, z, np,
                                                                                                   frame_of(p, ox, oy, oz), p->d, epx, epy, epz);
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// f3: one solve sharded over several GPUs; DESIGN.md section 9
+// ------------------------------------------------------------------------------------------------
+extern "C" int dks_poisson_set_shard(dks_poisson_plan *p, int rank, int nranks)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (nranks < 1 || nranks > kMaxRanks || (nranks & (nranks - 1)) || rank < 0 || rank >= nranks)
+        return fail(DKS_ERR_INVALID_ARG, "nranks must be a power of two in [1, %d] and 0 <= rank < nranks", kMaxRanks);
+    if (p->ws) return fail(DKS_ERR_INVALID_ARG, "dks_poisson_set_shard must be called before the workspace is attached / before dks_greens_setup");
+    if (nranks > 1) {
+        if (!(p->fast[0] && p->fast[1] && p->fast[2]))
+            return fail(DKS_ERR_INVALID_ARG, "a sharded solve needs nx, ny, nz in [32, 256] (register-resident passes on every axis)");
+        if (p->d.ny / nranks < 1 || p->d.nz / nranks < 1) return fail(DKS_ERR_INVALID_ARG, "more ranks than rows");
+        if (p->max_batch != 1 || p->slab != p->d.nz + 1) return fail(DKS_ERR_INVALID_ARG, "sharding excludes batches and slabs");
+    }
+    p->rank = rank; p->nranks = nranks;
+    p->ny_loc = p->d.ny / nranks; p->y0 = rank * p->ny_loc;
+    const int split = p->d.nz / nranks;                       // the last rank also takes plane nz
+    p->kz0 = rank * split; p->planes_loc = split + (rank == nranks - 1 ? 1 : 0);
+    p->pdl = p->pdl && nranks == 1;
+    compute_layout(p);
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_shard_buffers(dks_poisson_plan *p, void **recv_p1, void **recv_p4)
+{
+    if (!p || !recv_p1 || !recv_p4) return fail(DKS_ERR_INVALID_ARG, "plan or output pointer is NULL");
+    if (p->nranks < 2 || !p->ws) return fail(DKS_ERR_NOT_SETUP, "call dks_poisson_set_shard and attach the workspace (or dks_greens_setup) first");
+    *recv_p1 = p->A; *recv_p4 = p->A2;
+    return DKS_OK;
+}
+
+extern "C" int dks_poisson_set_peers(dks_poisson_plan *p, void *const *recv_p1_of_rank, void *const *recv_p4_of_rank)
+{
+    if (!p || !recv_p1_of_rank || !recv_p4_of_rank) return fail(DKS_ERR_INVALID_ARG, "plan or pointer table is NULL");
+    if (p->nranks < 2 || !p->ws) return fail(DKS_ERR_NOT_SETUP, "call dks_poisson_set_shard and attach the workspace (or dks_greens_setup) first");
+    int l1 = 0, l2 = 0;
+    while ((1 << l1) < p->d.nz / p->nranks) ++l1;
+    while ((1 << l2) < p->ny_loc) ++l2;
+    for (int r = 0; r < p->nranks; ++r) {
+        if (!recv_p1_of_rank[r] || !recv_p4_of_rank[r]) return fail(DKS_ERR_INVALID_ARG, "peer buffer of rank %d is NULL", r);
+        p->peers1.base[r] = static_cast<cplx *>(recv_p1_of_rank[r]);
+        p->peers2.base[r] = static_cast<cplx *>(recv_p4_of_rank[r]);
+    }
+    if (p->peers1.base[p->rank] != p->A || p->peers2.base[p->rank] != p->A2)
+        return fail(DKS_ERR_INVALID_ARG, "entry %d of the tables must be this rank's own buffers (dks_poisson_shard_buffers)", p->rank);
+    p->peers1.nranks = p->peers2.nranks = p->nranks;
+    p->peers1.lsplit = l1; p->peers1.first = p->y0; p->peers1.pitch = p->d.ny;
+    p->peers2.lsplit = l2; p->peers2.first = p->kz0; p->peers2.pitch = p->ny_loc;
+    p->peers_set = true;
+    return DKS_OK;
+}
+
+template <int A>
+static void shard_launch_p1(const dks_poisson_plan *p, const double *rho, cudaStream_t st)
+{
+    MeshDims d = p->d;
+    d.ny = p->ny_loc;                                          // this rank's y rows only
+    const int T = R16Geom<A>::THREADS, tiles = d.nx / (2 * kCols) * d.ny;
+    const int per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
+    p1_z_r2c_r16<A, false, true><<<std::min(tiles, p->sm_count * per_sm), T, P1Geom<A>::SMEM, st>>>(rho, nullptr, d, 1, p->tw1[2], p->tw[2], p->peers1);
+}
+
+template <int A>
+static void shard_launch_p4(const dks_poisson_plan *p, cudaStream_t st)
+{
+    p4_y_inv_r16<A, false, true><<<dim3(p->d.nx / kCols, p->planes_loc), R16Geom<A>::THREADS, R16Geom<A>::SMEM, st>>>(
+        p->B, nullptr, p->d, 0, p->tw1[1], p->tw[1], p->peers2);
+}
+
+// phase 1: P1 on this rank's y slab, rows stored to the owners of their kz planes
+// phase 2: P2, P3, P4 on this rank's kz slab, P4's rows stored to the owners of their y rows
+// phase 3: P5 on this rank's y slab
+// Between the phases every rank must have finished the previous phase (the caller's barrier: an NCCL barrier on the same
+// stream, or stream order when the ranks are emulated on one device).
+extern "C" int dks_poisson_solve_shard(dks_poisson_plan *p, int phase, const double *rho_loc, double *phi_loc, void *stream)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (p->nranks < 2 || !p->peers_set) return fail(DKS_ERR_NOT_SETUP, "call dks_poisson_set_shard, dks_greens_setup and dks_poisson_set_peers first");
+    if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve_shard");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (p->setup_pending && st != p->setup_used) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+    const MeshDims d = p->d;
+    switch (phase) {
+    case 1:
+        if (!rho_loc || reinterpret_cast<uintptr_t>(rho_loc) % 16) return fail(DKS_ERR_INVALID_ARG, "rho_loc is NULL or not 16-byte aligned");
+        switch (p->r16A[2]) {
+#define X(A_) case A_: shard_launch_p1<A_>(p, rho_loc, st); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+        break;
+    case 2: {
+        dks_poisson_plan::Step s2 = { 2, 0, p->planes_loc }, s3 = { 3, p->kz0, p->planes_loc };
+        launch_r16(s2, p, nullptr, nullptr, 1, st);            // reads A1 (= p->A, local planes), writes B
+        launch_r16(s3, p, nullptr, nullptr, 1, st);            // Ghat planes kz0 ..
+        switch (p->r16A[1]) {
+#define X(A_) case A_: shard_launch_p4<A_>(p, st); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+        break;
+    }
+    case 3: {
+        if (!phi_loc || reinterpret_cast<uintptr_t>(phi_loc) % 16) return fail(DKS_ERR_INVALID_ARG, "phi_loc is NULL or not 16-byte aligned");
+        MeshDims dl = d;
+        dl.ny = p->ny_loc;
+        switch (p->r16A[2]) {
+#define X(A_) case A_: p5_z_c2r_r16<A_, false><<<dim3(d.nx / (2 * kCols), dl.ny, 1), R16Geom<A_>::THREADS, R16Geom<A_>::SMEM, st>>>(p->A2, phi_loc, dl, p->tw1[2], p->tw[2]); break;
+            DKS_FOR_EACH_A(X)
+#undef X
+        }
+        break;
+    }
+    default: return fail(DKS_ERR_INVALID_ARG, "phase must be 1, 2 or 3");
+    }
     DKS_CUDA(cudaGetLastError());
     return DKS_OK;
 }

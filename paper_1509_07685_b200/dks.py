@@ -49,6 +49,10 @@ SYMBOLS = {
     "dks_deposit_cic": (_i, [_vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp]),
     "dks_gradient": (_i, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dks_gather_field": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
+    "dks_poisson_set_shard": (_i, [_vp, _i, _i]),
+    "dks_poisson_shard_buffers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "dks_poisson_set_peers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "dks_poisson_solve_shard": (_i, [_vp, _i, _vp, _vp, _vp]),
     "dks_last_error": (C.c_char_p, []),
 }
 
@@ -209,6 +213,26 @@ def dks_gradient(plan, phi, ex, ey, ez, stream=None):
 def dks_gather_field(plan, ex, ey, ez, x, y, z, np_, origin, epx, epy, epz, stream=None):
     return _check(lib.dks_gather_field(plan, _ptr(ex), _ptr(ey), _ptr(ez), _ptr(x), _ptr(y), _ptr(z), int(np_),
                                        *(float(v) for v in origin), _ptr(epx), _ptr(epy), _ptr(epz), stream), "dks_gather_field")
+
+
+def dks_poisson_set_shard(plan, rank, nranks):
+    return _check(lib.dks_poisson_set_shard(plan, int(rank), int(nranks)), "dks_poisson_set_shard")
+
+
+def dks_poisson_shard_buffers(plan):
+    a, b = _vp(), _vp()
+    _check(lib.dks_poisson_shard_buffers(plan, C.byref(a), C.byref(b)), "dks_poisson_shard_buffers")
+    return a.value, b.value
+
+
+def dks_poisson_set_peers(plan, recv_p1_of_rank, recv_p4_of_rank):
+    n = len(recv_p1_of_rank)
+    t1, t2 = (_vp * n)(*recv_p1_of_rank), (_vp * n)(*recv_p4_of_rank)
+    return _check(lib.dks_poisson_set_peers(plan, t1, t2), "dks_poisson_set_peers")
+
+
+def dks_poisson_solve_shard(plan, phase, rho_loc, phi_loc, stream=None):
+    return _check(lib.dks_poisson_solve_shard(plan, int(phase), _ptr(rho_loc), _ptr(phi_loc), stream), "dks_poisson_solve_shard")
 
 
 # ---- convenience wrapper (still marshalling only) ---------------------------------------------------
