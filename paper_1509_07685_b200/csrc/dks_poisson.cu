@@ -19,6 +19,7 @@
 #include "../../include/dks_poisson.h"
 #include "dks_passes_generic.cuh"
 #include "dks_passes_r16.cuh"
+#include "dks_passes_big.cuh"
 #include "dks_greens_r16.cuh"
 #include "dks_field_ops.cuh"
 
@@ -67,6 +68,8 @@ struct dks_poisson_plan {
     cplx *tw1[3] = { nullptr, nullptr, nullptr };
     std::vector<cplx> tw1_host[3];
     bool fast[5] = { false, false, false, false, false };   // pass P1..P5 uses the r16 kernel
+    int big[5] = { 0, 0, 0, 0, 0 };     // pass P1..P5 uses the long-line kernel with this padded length (1024 / 2048), else 0
+    int bigL[3] = { 0, 0, 0 };          // per axis: 2n if n = 512 or 1024
     void *ws = nullptr;                 // workspace base
     size_t ws_bytes = 0;
     bool ws_owned = false;
@@ -226,6 +229,10 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
                 }
     }
     // P1/P5 run along z and need 16 real columns per CTA; P2/P4 along y; P3 along x (nx = 256 only)
+    for (int a = 0; a < 3; ++a) p->bigL[a] = (ns[a] == 512 || ns[a] == 1024) ? 2 * ns[a] : 0;
+    p->big[0] = p->big[4] = (p->bigL[2] && nx >= 2 * (p->bigL[2] == 1024 ? BigGeom<1024>::W : BigGeom<2048>::W)) ? p->bigL[2] : 0;
+    p->big[1] = p->big[3] = p->bigL[1];
+    p->big[2] = p->bigL[0];
     p->fast[0] = p->fast[4] = p->r16A[2] != 0 && nx >= 16;
     p->fast[1] = p->fast[3] = p->r16A[1] != 0;
     p->fast[2] = p->r16A[0] != 0;
@@ -371,6 +378,34 @@ static void launch_r16(const dks_poisson_plan::Step &s, const dks_poisson_plan *
     }
 }
 
+template <int L>
+static void launch_big(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
+                       int nb, cudaStream_t st)
+{
+    typedef BigGeom<L> G;
+    const MeshDims d = p->d;
+    switch (s.pass) {
+    case 1: p1_z_r2c_big<L><<<dim3(d.nx / (2 * G::W), d.ny, nb), G::THREADS, G::SMEM, st>>>(rho, p->A, d, p->tw[2]); break;
+    case 2: p2_y_fwd_big<L><<<dim3(d.nx / G::W, s.planes * nb), G::THREADS, G::SMEM, st>>>(p->A, p->B, d, s.kz0, p->tw[1]); break;
+    case 3: p3_x_conv_big<L><<<(unsigned)((size_t)s.planes * nb * 2 * d.ny / G::W), G::THREADS, P3BigGeom<L>::SMEM, st>>>(p->B, p->G, d, s.kz0, p->tw[0]); break;
+    case 4: p4_y_inv_big<L><<<dim3(d.nx / G::W, s.planes * nb), G::THREADS, G::SMEM, st>>>(p->B, p->A, d, s.kz0, p->tw[1]); break;
+    case 5: p5_z_c2r_big<L><<<dim3(d.nx / (2 * G::W), d.ny, nb), G::THREADS, G::SMEM, st>>>(p->A, phi, d, p->tw[2]); break;
+    }
+}
+
+template <int L>
+static int big_set_attributes()
+{
+    typedef BigGeom<L> G;
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(p3_x_conv_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, P3BigGeom<L>::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM));
+    DKS_CUDA(cudaFuncSetAttribute(greens_axis_big<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEMX));
+    return DKS_OK;
+}
+
 static void launch_generic(const dks_poisson_plan::Step &s, const dks_poisson_plan *p, const double *rho, double *phi,
                            int nb, cudaStream_t st)
 {
@@ -430,6 +465,7 @@ static int ensure_device(dks_poisson_plan *p)
         DKS_CUDA(cudaFuncSetAttribute(greens_axis_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_lines));
         int rc = r16_set_attributes();
         if (rc) return rc;
+        if ((rc = big_set_attributes<1024>()) || (rc = big_set_attributes<2048>())) return rc;
         if (dev < 64) attributes_set[dev] = true;
     }
     DKS_CUDA(cudaEventCreateWithFlags(&p->ghat_free, cudaEventDisableTiming));
@@ -547,6 +583,9 @@ static int greens_setup_on(dks_poisson_plan *p, cudaStream_t st)
         greens_fill_kernel<<<grd, blk, 0, st>>>(p->G, d, p->hx, p->hy, p->hz, coef, g0);
         long long nl = (long long)(d.ny + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.nx * (W + 1) * sizeof(cplx);
+        if (p->bigL[0] == 1024) greens_axis_big<1024><<<(unsigned)((nl + 2 * BigGeom<1024>::W - 1) / (2 * BigGeom<1024>::W)), BigGeom<1024>::THREADS, BigGeom<1024>::SMEMX, st>>>(p->G, 1, d.ny + 1, pitch, d.nz + 1, plane, 1.0, p->tw[0]);
+        else if (p->bigL[0] == 2048) greens_axis_big<2048><<<(unsigned)((nl + 2 * BigGeom<2048>::W - 1) / (2 * BigGeom<2048>::W)), BigGeom<2048>::THREADS, BigGeom<2048>::SMEMX, st>>>(p->G, 1, d.ny + 1, pitch, d.nz + 1, plane, 1.0, p->tw[0]);
+        else
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nx, d.lx, W, 1, d.ny + 1, pitch,
                                                                                    d.nz + 1, plane, 1.0, p->tw[0]);
     }
@@ -560,6 +599,9 @@ static int greens_setup_on(dks_poisson_plan *p, cudaStream_t st)
     } else {
         long long nl = (long long)(d.nx + 1) * (d.nz + 1);
         size_t sm = (size_t)2 * d.ny * (W + 1) * sizeof(cplx);
+        if (p->bigL[1] == 1024) greens_axis_big<1024><<<(unsigned)((nl + 2 * BigGeom<1024>::W - 1) / (2 * BigGeom<1024>::W)), BigGeom<1024>::THREADS, BigGeom<1024>::SMEMX, st>>>(p->G, pitch, d.nx + 1, 1, d.nz + 1, plane, 1.0, p->tw[1]);
+        else if (p->bigL[1] == 2048) greens_axis_big<2048><<<(unsigned)((nl + 2 * BigGeom<2048>::W - 1) / (2 * BigGeom<2048>::W)), BigGeom<2048>::THREADS, BigGeom<2048>::SMEMX, st>>>(p->G, pitch, d.nx + 1, 1, d.nz + 1, plane, 1.0, p->tw[1]);
+        else
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.ny, d.ly, W, pitch, d.nx + 1, 1,
                                                                                    d.nz + 1, plane, 1.0, p->tw[1]);
     }
@@ -572,6 +614,9 @@ static int greens_setup_on(dks_poisson_plan *p, cudaStream_t st)
     } else {
         long long nl = (long long)(d.nx + 1) * (d.ny + 1);
         size_t sm = (size_t)2 * d.nz * (W + 1) * sizeof(cplx);
+        if (p->bigL[2] == 1024) greens_axis_big<1024><<<(unsigned)((nl + 2 * BigGeom<1024>::W - 1) / (2 * BigGeom<1024>::W)), BigGeom<1024>::THREADS, BigGeom<1024>::SMEMX, st>>>(p->G, plane, d.nx + 1, 1, d.ny + 1, pitch, scale, p->tw[2]);
+        else if (p->bigL[2] == 2048) greens_axis_big<2048><<<(unsigned)((nl + 2 * BigGeom<2048>::W - 1) / (2 * BigGeom<2048>::W)), BigGeom<2048>::THREADS, BigGeom<2048>::SMEMX, st>>>(p->G, plane, d.nx + 1, 1, d.ny + 1, pitch, scale, p->tw[2]);
+        else
         greens_axis_kernel<<<(unsigned)((nl + 2 * W - 1) / (2 * W)), 256, sm, st>>>(p->G, d.nz, d.lz, W, plane, d.nx + 1, 1,
                                                                                    d.ny + 1, pitch, scale, p->tw[2]);
     }
@@ -632,7 +677,8 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     static const char *names[5] = { "p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic",
                                     "p4_y_inv_generic", "p5_z_c2r_generic" };
     static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
-    return p->fast[pass - 1] ? fast_names[pass - 1] : names[pass - 1];
+    static const char *big_names[5] = { "p1_z_r2c_big", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_big" };
+    return p->fast[pass - 1] ? fast_names[pass - 1] : p->big[pass - 1] ? big_names[pass - 1] : names[pass - 1];
 }
 
 // Events of one profiled solve: one before every launch of the launch list and one after the last.
@@ -720,6 +766,8 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
         const dks_poisson_plan::Step &s = p->steps[i];
         if (prof) DKS_CUDA(cudaEventRecord(ev[i], st));
         if (p->fast[s.pass - 1]) launch_r16(s, p, rho, phi, nb, st);
+        else if (p->big[s.pass - 1] == 1024) launch_big<1024>(s, p, rho, phi, nb, st);
+        else if (p->big[s.pass - 1] == 2048) launch_big<2048>(s, p, rho, phi, nb, st);
         else launch_generic(s, p, rho, phi, nb, st);
         // a later rebuild of Ghat on the setup stream must not overtake this solve's last P3
         if (s.pass == 3 && last_p3(p, i) && st != p->setup_used && !capturing) {

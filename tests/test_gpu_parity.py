@@ -133,7 +133,7 @@ def test_paper_table1_shapes(torch_cuda, dks, oracle, workloads, n):
 
 
 def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
-    # 512x512x256 (padded 1024x1024x512): x and y run the generic passes (n = 512), z the register-resident ones.
+    # 512x512x256 (padded 1024x1024x512): x and y run the long-line passes (n = 512, dks_passes_big.cuh), z the register-resident ones.
     # Checked against direct summation of Eq. (2) at sampled nodes (one pass over rho per node).
     n, h = (512, 512, 256), (1e-4, 1e-4, 2e-4)
     rho = workloads.random_rho(n, seed=99, signed=False)
@@ -276,6 +276,8 @@ def test_greens_point_charge_at_origin_returns_G(torch_cuda, dks, oracle):
 
 # ---- step a0 directly: the Green's octant of dks_greens_setup against the oracle's FT{Gt} ----
 @pytest.mark.parametrize("n,h,g0", [((16, 8, 32), (1e-3, 2e-3, 5e-4), None),           # generic x, y; r16 z
+                                     ((512, 16, 8), (5e-5, 1e-3, 1e-3), None),            # long-line x (greens_axis_big)
+                                     ((8, 1024, 16), (1e-3, 2e-5, 1e-3), None),           # long-line y
                                      ((32, 64, 16), (2e-4, 3e-4, 1e-4), 7.5e12),         # r16 x, y; generic z
                                      ((128, 32, 64), (1e-4, 2e-4, 4e-4), None),
                                      ((256, 16, 8), (1e-4, 1e-3, 1e-3), None),
@@ -500,6 +502,19 @@ def test_caller_owned_and_plan_owned_workspace(torch_cuda, dks, oracle, workload
         assert e.value.status == dks.DKS_ERR_NOT_SETUP
     finally:
         dks.dks_poisson_plan_destroy(h_)
+
+
+def test_long_line_passes_are_selected(dks):
+    cases = {(64, 64, 512): ["p1_z_r2c_big", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_big"],
+             (512, 512, 256): ["p1_z_r2c_r16", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_r16"],
+             (8, 1024, 1024): ["p1_z_r2c_big", "p2_y_fwd_big", "p3_x_conv_generic", "p4_y_inv_big", "p5_z_c2r_big"],
+             (8, 8, 512): ["p1_z_r2c_generic", "p2_y_fwd_generic", "p3_x_conv_generic", "p4_y_inv_generic", "p5_z_c2r_generic"]}
+    for n, names in cases.items():
+        h_ = dks.dks_poisson_plan_create(*n, 1e-3, 1e-3, 1e-3)
+        try:
+            assert [dks.dks_poisson_pass_name(h_, i) for i in range(1, 6)] == names
+        finally:
+            dks.dks_poisson_plan_destroy(h_)
 
 
 def test_pass_times_and_names(torch_cuda, dks, workloads):
