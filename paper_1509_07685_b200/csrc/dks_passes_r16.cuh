@@ -1,4 +1,5 @@
-// Specialised passes for mesh extents n = 16 A, A in {2,4,8,16} (n = 32..256) on the pass's own axis.
+// Specialised passes for mesh extents n = 16 A, A in {1,2,4,8,16} (n = 16..256) on the pass's own axis (A = 1: the whole
+// sub-transform is one thread's radix-16, the exchange degenerates to the identity).
 // Same buffers and layouts as the generic passes (dks_passes_generic.cuh), so any pass may use
 // either variant:
 //
@@ -186,7 +187,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     const int tid = threadIdx.x, lane = tid & 31, c = tid & 7, p = (tid >> 3) & 1;
     const int a = p1_a_of<A>(p, (tid >> 4) & 1, tid >> 5);
     const bool a0 = a == 0 && p == 0;                     // holds k = 0 and k = n, mirrors inside its own registers
-    const int partner = (p == 0 && tid < 32) ? lane : lane ^ 16;
+    const int partner = (A == 1 || (p == 0 && tid < 32)) ? lane : lane ^ 16;
     const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny * nb;   // nb meshes back to back
     auto prefetch = [&](int t) {
         const int yy = t / xtiles, y = yy % ny;
@@ -331,13 +332,13 @@ constexpr int kP3Smem = kP3Warps * kP3SmemPerWarp;
 
 template <int A>
 struct P3Ex {
-    static constexpr int SWZ = A >= 4 ? 3 : 1;
+    static constexpr int SWZ = A >= 4 ? 3 : A - 1;
     static constexpr int OFFP = A >= 4 ? 4 : 2;        // elements
     static constexpr int OFFJ = 4;                     // keeps region (j, 1) clear of region (j + 1, 0)
     static constexpr int GROW = (16 * A + 2) * 8;      // bytes of a Ghat row that are needed (n + 1 doubles, rounded to 16 B)
-    static constexpr int GSTR = A == 2 ? 36 : 16 * A + 8;   // shared-memory row stride (doubles): rows of a half-warp on distinct banks
+    static constexpr int GSTR = A == 1 ? 18 : A == 2 ? 36 : 16 * A + 8;   // shared-memory row stride (doubles): rows of a half-warp on distinct banks
     static_assert(GROW <= GSTR * 8 && (16 / A) * GSTR * 8 <= kP3GBytes, "Ghat stage");
-    static_assert((2 * (16 / A) * 16 * A + OFFP + (16 / A - 1) * OFFJ) * 16 <= kP3ExBytes, "exchange buffer");
+    static_assert(A == 1 || (2 * (16 / A) * 16 * A + OFFP + (16 / A - 1) * OFFJ) * 16 <= kP3ExBytes, "exchange buffer");   // A = 1 needs none
 };
 
 template <int A, bool PDL>
@@ -423,14 +424,16 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
         fft16<-1>(v);
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = cmul(v[k], tb[k]);
+        if (A > 1) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) ex[k * A + (a ^ (k & SWZ))] = v[k];
-        __syncwarp();
+            for (int k = 0; k < 16; ++k) ex[k * A + (a ^ (k & SWZ))] = v[k];
+            __syncwarp();
 #pragma unroll
-        for (int g = 0; g < G; ++g)
+            for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[(a + A * g) * A + (ap ^ (a & SWZ))];
-        fft_second<A, -1>(v);
+                for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[(a + A * g) * A + (ap ^ (a & SWZ))];
+            fft_second<A, -1>(v);
+        }
         // multiply by the real, even Green's transform
         mbar_wait(&bar[1], phase);
 #pragma unroll
@@ -442,14 +445,18 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
         if (lane == 0 && next < ngroups) fetch_ghat();
         advance();
         // inverse, transposed flow: radix-A, exchange back, conj tb, radix-16
-        fft_second_t<A, +1>(v);
+        if (A > 1) {
+            fft_second_t<A, +1>(v);
 #pragma unroll
-        for (int g = 0; g < G; ++g)
+            for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int ap = 0; ap < A; ++ap) ex[(a + A * g) * A + (ap ^ (a & SWZ))] = v[g * A + ap];
-        __syncwarp();
+                for (int ap = 0; ap < A; ++ap) ex[(a + A * g) * A + (ap ^ (a & SWZ))] = v[g * A + ap];
+            __syncwarp();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = cmulc(ex[k * A + (a ^ (k & SWZ))], tb[k]);
+            for (int k = 0; k < 16; ++k) v[k] = ex[k * A + (a ^ (k & SWZ))];
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = cmulc(v[k], tb[k]);
         fft16<+1>(v);
         if (p) parity_consts<+1>(v);
         // combine the parities (crop fused): y[m] = O_0[m] + w_L^-m O_1[m]; parity 0 keeps the even registers, parity 1 the odd ones

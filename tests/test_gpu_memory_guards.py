@@ -23,7 +23,7 @@ def guards_intact(torch, buf, numel):
     return bool(torch.all(buf[:GUARD] == SENTINEL)) and bool(torch.all(buf[GUARD + numel:] == SENTINEL))
 
 
-SHAPES = [(8, 8, 8), (16, 8, 32), (32, 16, 64), (64, 64, 16), (128, 32, 16), (256, 16, 8), (16, 256, 32), (8, 32, 256),
+SHAPES = [(8, 8, 8), (16, 8, 32), (16, 16, 64), (32, 16, 64), (64, 64, 16), (128, 32, 16), (256, 16, 8), (16, 256, 32), (8, 32, 256),
           (512, 8, 16), (8, 8, 1024), (16, 512, 8)]
 
 

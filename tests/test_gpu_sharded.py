@@ -61,7 +61,7 @@ def test_shard_refusals():
     finally:
         torch.cuda.synchronize()
         dks.dks_poisson_plan_destroy(h_)
-    g_ = dks.dks_poisson_plan_create(16, 64, 64, 1e-3, 1e-3, 1e-3)     # nx = 16 has no register-resident x pass
+    g_ = dks.dks_poisson_plan_create(8, 64, 64, 1e-3, 1e-3, 1e-3)      # nx = 8 has no register-resident x pass
     try:
         with pytest.raises(dks.DksError):
             dks.dks_poisson_set_shard(g_, 0, 2)
