@@ -408,6 +408,14 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     cplx tb[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) tb[k] = __ldg(&tw1[p * N + k * A + a]);
+    // the XOR swizzle only touches the two low bits of the column: four lane-dependent bases per direction, everything
+    // else is an immediate offset (keeps the address arithmetic out of the loop)
+    cplx *exw[4], *exr[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        exw[c] = ex + (a ^ (c & SWZ));                        // + k A,  c = k & 3
+        exr[c] = ex + a * A + ((c ^ a) & SWZ);                // + A A g + (ap & ~SWZ),  c = ap & 3
+    }
 
     unsigned phase = 0;
     for (; grp < ngroups; grp += stride, phase ^= 1) {
@@ -426,12 +434,12 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
         for (int k = 0; k < 16; ++k) v[k] = cmul(v[k], tb[k]);
         if (A > 1) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) ex[k * A + (a ^ (k & SWZ))] = v[k];
+            for (int k = 0; k < 16; ++k) exw[k & 3][k * A] = v[k];
             __syncwarp();
 #pragma unroll
             for (int g = 0; g < G; ++g)
 #pragma unroll
-                for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[(a + A * g) * A + (ap ^ (a & SWZ))];
+                for (int ap = 0; ap < A; ++ap) v[g * A + ap] = exr[ap & 3][A * A * g + (ap & ~SWZ)];
             fft_second<A, -1>(v);
         }
         // multiply by the real, even Green's transform
@@ -450,10 +458,10 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 #pragma unroll
             for (int g = 0; g < G; ++g)
 #pragma unroll
-                for (int ap = 0; ap < A; ++ap) ex[(a + A * g) * A + (ap ^ (a & SWZ))] = v[g * A + ap];
+                for (int ap = 0; ap < A; ++ap) exr[ap & 3][A * A * g + (ap & ~SWZ)] = v[g * A + ap];
             __syncwarp();
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = ex[k * A + (a ^ (k & SWZ))];
+            for (int k = 0; k < 16; ++k) v[k] = exw[k & 3][k * A];
         }
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = cmulc(v[k], tb[k]);
