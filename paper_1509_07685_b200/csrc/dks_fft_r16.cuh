@@ -235,6 +235,76 @@ __device__ __forceinline__ void twiddle_between_s(cplx (&v)[16], const cplx *T, 
     for (int k = 0; k < 16; ++k) v[k] = SIGN < 0 ? cmul(v[k], T[k * A + a]) : cmulc(v[k], T[k * A + a]);
 }
 
+// ---- twiddle AFTER the exchange ----------------------------------------------------------------
+// The between-step twiddle commutes with the exchange: the thread that holds sub-transform index k = a + A g after the
+// exchange multiplies its value from pre-exchange thread a' by T[k A + a'], i.e. by A consecutive table entries per g.
+// The strided passes issue these loads right before the exchange barrier, when v[] is dead, so their latency hides
+// behind the barrier, and for A = 16 the multiplication is folded into the first butterfly layer of the second
+// radix-16 (fft16_tw): x0 + t x2 is 4 FMAs, x0 - t x2 = 2 x0 - (x0 + t x2) two more, which saves 4 of the 32 (28)
+// instructions of a 4-point butterfly with 4 (3) twiddled inputs.
+template <int A>
+__device__ __forceinline__ void load_tw_post(cplx (&t)[16], const cplx *__restrict__ T, int a)
+{
+    constexpr int G = 16 / A;
+    if constexpr (A > 1) {                                // A = 1: every table entry is 1 (fft_second_tw skips the product)
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int ap = 0; ap < A; ++ap) t[g * A + ap] = __ldg(&T[(a + A * g) * A + ap]);
+    }
+}
+
+// u + t x  (SIGN < 0) or u + conj(t) x  (SIGN > 0)
+template <int SIGN>
+__device__ __forceinline__ cplx cfma_tw(cplx t, cplx x, cplx u)
+{
+    const double ty = SIGN < 0 ? t.y : -t.y;
+    return cmake(fma(-ty, x.y, fma(t.x, x.x, u.x)), fma(ty, x.x, fma(t.x, x.y, u.y)));
+}
+template <int SIGN>
+__device__ __forceinline__ cplx cmul_tw(cplx x, cplx t) { return SIGN < 0 ? cmul(x, t) : cmulc(x, t); }
+// 2 a - b
+__device__ __forceinline__ cplx ctwice_minus(cplx a, cplx b) { return cmake(fma(2.0, a.x, -b.x), fma(2.0, a.y, -b.y)); }
+
+// bfly4 on (t0 x0, t1 x1, t2 x2, t3 x3) (conjugated twiddles for SIGN > 0); UNIT0: t0 = 1
+template <int SIGN, bool UNIT0>
+__device__ __forceinline__ void bfly4_tw(cplx &x0, cplx &x1, cplx &x2, cplx &x3, cplx t0, cplx t1, cplx t2, cplx t3)
+{
+    const cplx y0 = UNIT0 ? x0 : cmul_tw<SIGN>(x0, t0);
+    const cplx apc = cfma_tw<SIGN>(t2, x2, y0), amc = ctwice_minus(y0, apc);
+    const cplx y1 = cmul_tw<SIGN>(x1, t1);
+    const cplx bpd = cfma_tw<SIGN>(t3, x3, y1), bmd = mul_si<SIGN>(ctwice_minus(y1, bpd));
+    x0 = cadd(apc, bpd);
+    x1 = cadd(amc, bmd);
+    x2 = csub(apc, bpd);
+    x3 = csub(amc, bmd);
+}
+
+// fft16 of (t[i] v[i]); UNIT0: t[0] = 1
+template <int SIGN, bool UNIT0>
+__device__ __forceinline__ void fft16_tw(cplx (&v)[16], const cplx (&t)[16])
+{
+    bfly4_tw<SIGN, UNIT0>(v[0], v[4], v[8], v[12], t[0], t[4], t[8], t[12]);
+#pragma unroll
+    for (int n0 = 1; n0 < 4; ++n0) bfly4_tw<SIGN, false>(v[n0], v[n0 + 4], v[n0 + 8], v[n0 + 12], t[n0], t[n0 + 4], t[n0 + 8], t[n0 + 12]);
+    fft16_tail<SIGN>(v);
+}
+
+// second step of the four-step transform with the twiddles t[] (load_tw_post) applied to its inputs
+template <int A, int SIGN, bool UNIT0>
+__device__ __forceinline__ void fft_second_tw(cplx (&v)[16], const cplx (&t)[16])
+{
+    if (A == 16) {
+        fft16_tw<SIGN, UNIT0>(v, t);
+        return;
+    }
+    if (A > 1) {                                          // A = 1: every table entry is 1
+#pragma unroll
+        for (int i = 0; i < 16; ++i) v[i] = cmul_tw<SIGN>(v[i], t[i]);
+    }
+    fft_second<A, SIGN>(v);
+}
+
 // cos, sin of 2 pi m / 32, m = 0..15
 __device__ __forceinline__ constexpr double cos32(int m)
 {

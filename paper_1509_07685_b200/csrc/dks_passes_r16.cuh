@@ -37,6 +37,33 @@ struct PeerTable {
     int first;               // P1: first global y row of this rank's slab;  P4: first global kz plane of this rank's slab
     int pitch;               // P1: global ny (rows per plane in the receiver);  P4: y rows per rank (rows per plane in the receiver)
 };
+#ifndef DKS_TW_POST
+#define DKS_TW_POST 1
+#endif
+#ifndef DKS_P5_LDCACHED
+#define DKS_P5_LDCACHED 1
+#endif
+#ifndef DKS_P5_DIRECT
+#define DKS_P5_DIRECT 1
+#endif
+#ifndef DKS_P1_BULK
+#define DKS_P1_BULK 1      // P1's stage completes on an mbarrier (no block barrier at the top of a tile)
+#endif
+#ifndef DKS_STAGE_BULK
+#define DKS_STAGE_BULK 0   // 1: one 128-byte cp.async.bulk per row instead of 16-byte cp.async (measured slower)
+#endif
+#if DKS_P1_BULK && !DKS_TW_POST
+#error DKS_P1_BULK needs DKS_TW_POST
+#endif
+#ifndef DKS_P4_TW_POST
+#define DKS_P4_TW_POST false
+#endif
+#ifndef DKS_P5_TW_POST
+#define DKS_P5_TW_POST true
+#endif
+#ifndef DKS_PDL_LATE
+#define DKS_PDL_LATE 0
+#endif
 #ifndef DKS_R16_OCC
 #define DKS_R16_OCC 512
 #endif
@@ -58,6 +85,19 @@ __device__ __forceinline__ void strided_forward(cplx (&v)[16], cplx *ex, int c, 
 {
     if (p) parity_consts<-1>(v);
     fft16<-1>(v);
+#if DKS_TW_POST
+#pragma unroll
+    for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+    cplx t[16];
+    load_tw_post<A>(t, tw1 + p * 16 * A, a);             // in flight across the barrier (dks_fft_r16.cuh)
+    __syncthreads();
+    constexpr int G = 16 / A;
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
+    fft_second_tw<A, -1, true>(v, t);                    // regions 0 and 1 have T = 1 at a' = 0
+#else
     twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
@@ -68,14 +108,28 @@ __device__ __forceinline__ void strided_forward(cplx (&v)[16], cplx *ex, int c, 
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
     fft_second<A, -1>(v);
+#endif
 }
 
 // inverse: v[b] = X[2 (a + A b) + p] on entry; on exit v[r] = IFFT_n(X_p)[a + A r] (* w_L^-(a + A r) if p)
-template <int A>
+template <int A, bool POST>
 __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, int p, int a,
                                                 const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     fft16<+1>(v);
+    if (POST) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+    cplx t[16];
+    load_tw_post<A>(t, tw1 + p * 32 * A, a);
+    __syncthreads();
+    constexpr int G = 16 / A;
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
+    fft_second_tw<A, +1, false>(v, t);                   // region 2 carries the thread constant w_L^(k mod A): no unit entry
+    } else {
     twiddle_between<A, +1>(v, tw1 + p * 32 * A, a);
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
@@ -86,6 +140,7 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
     fft_second<A, +1>(v);
+    }
     if (p) parity_consts<+1>(v);
 }
 
@@ -102,13 +157,14 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;          // kz: plane within the slab
     const size_t x = (size_t)blockIdx.x * kCols + c;
     if (PDL) {
-        pdl_trigger();
+        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
     strided_forward<A>(v, ex, c, p, a, tw1, tw2);
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
 #pragma unroll
     for (int r = 0; r < 16; ++r)
         stg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * r) + p) * nx + x], v[r]);
@@ -127,16 +183,17 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
     const size_t x = (size_t)blockIdx.x * kCols + c;
     if (PDL) {
-        pdl_trigger();
+        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b)
         v[b] = ldg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * b) + p) * nx + x]);
-    strided_inverse<A>(v, ex, c, p, a, tw1, tw2);
+    strided_inverse<A, DKS_P4_TW_POST>(v, ex, c, p, a, tw1, tw2);
     cplx out[8];
     combine_parities<8>(v, p, out);
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int yrow = a + A * (i + 8 * p);
@@ -164,7 +221,7 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
 template <int A>
 struct P1Geom {
     static constexpr int STAGE = 16 * A * kCols * (int)sizeof(cplx);     // N rows x 8 packed pairs
-    static constexpr int SMEM = R16Geom<A>::SMEM + STAGE;
+    static constexpr int SMEM = R16Geom<A>::SMEM + STAGE + 16;             // + two mbarriers
 };
 
 // thread -> sub-transform index a such that mirror partners are lane ^ 16 (or the lane itself)
@@ -181,7 +238,7 @@ __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
 p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d, int nb,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2, PeerTable T)
 {
-    extern __shared__ cplx ex[];
+    extern __shared__ __align__(128) cplx ex[];
     constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
     cplx *stage = ex + L * kCols;
     const int tid = threadIdx.x, lane = tid & 31, c = tid & 7, p = (tid >> 3) & 1;
@@ -189,6 +246,30 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     const bool a0 = a == 0 && p == 0;                     // holds k = 0 and k = n, mirrors inside its own registers
     const int partner = (A == 1 || (p == 0 && tid < 32)) ? lane : lane ^ 16;
     const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny * nb;   // nb meshes back to back
+#if DKS_P1_BULK
+    uint64_t *bar = reinterpret_cast<uint64_t *>(stage + N * kCols);      // [0] stage filled, [1] exchange buffer read
+    if (tid == 0) {
+        mbar_init(&bar[0], DKS_STAGE_BULK ? 1 : THREADS);
+        mbar_init(&bar[1], THREADS);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    auto prefetch = [&](int t) {
+        const int yy = t / xtiles, y = yy % ny;
+        const double *src = rho + (size_t)(yy / ny) * N * ny * nx + (size_t)y * nx + (size_t)(t % xtiles) * 2 * kCols;
+#if DKS_STAGE_BULK
+        bulk_g2s(&stage[tid * kCols], &src[(size_t)tid * ny * nx], kCols * sizeof(cplx), &bar[0]);  // thread = input row z: 128 B
+#else
+#pragma unroll
+        for (int i = 0; i < N * kCols / THREADS; ++i) {
+            const int idx = tid + i * THREADS;
+            cp_async16(&stage[idx], &src[(size_t)(idx >> 3) * ny * nx + 2 * (idx & 7)]);
+        }
+        cp_async_mbar_arrive(&bar[0]);
+#endif
+    };
+    unsigned phase = 0;
+#else
     auto prefetch = [&](int t) {
         const int yy = t / xtiles, y = yy % ny;
         const double *src = rho + (size_t)(yy / ny) * N * ny * nx;
@@ -200,13 +281,22 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         }
         cp_async_commit();
     };
+#endif
     int t = blockIdx.x;
     if (PDL) {
-        pdl_trigger();
+        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();                                       // A is still being read by the previous solve's P5
     }
+#if DKS_P1_BULK
+    if (t < tiles) {
+        if (DKS_STAGE_BULK && tid == 0) mbar_expect_tx(&bar[0], N * kCols * sizeof(cplx));
+        prefetch(t);
+    }
+    for (; t < tiles; t += gridDim.x, phase ^= 1) {
+#else
     if (t < tiles) prefetch(t);
     for (; t < tiles; t += gridDim.x) {
+#endif
         const int yy = t / xtiles, y = yy % ny;
         const size_t xoff = (size_t)(t % xtiles) * 2 * kCols + 2 * c;
         cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx + (size_t)y * nx + xoff;
@@ -216,14 +306,41 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
             const int o = min(k >> T.lsplit, T.nranks - 1);
             return T.base[o] + ((size_t)(k - (o << T.lsplit)) * T.pitch + T.first + y) * nx + xoff;
         };
+#if DKS_P1_BULK
+        mbar_wait(&bar[0], phase);                        // stage complete
+#else
         cp_async_wait_all();
         __syncthreads();                                  // stage complete; last tile's exchange reads done
+#endif
         cplx v[16];
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[(a + A * b) * kCols + c];
         // ---- strided_forward, with the prefetch of the next tile issued once the stage is consumed
         if (p) parity_consts<-1>(v);
         fft16<-1>(v);
+#if DKS_TW_POST
+#if DKS_P1_BULK
+        if (t != (int)blockIdx.x) mbar_wait(&bar[1], phase ^ 1);          // the last tile's exchange reads are done
+#endif
+#pragma unroll
+        for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+        cplx twp[16];
+        load_tw_post<A>(twp, tw1 + p * 16 * A, a);
+#if DKS_P1_BULK
+        if (DKS_STAGE_BULK && tid == 0 && t + (int)gridDim.x < tiles) mbar_expect_tx(&bar[0], N * kCols * sizeof(cplx));
+#endif
+        __syncthreads();
+        if (t + (int)gridDim.x < tiles) prefetch(t + gridDim.x);
+        constexpr int G = 16 / A;
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
+#if DKS_P1_BULK
+        mbar_arrive(&bar[1]);
+#endif
+        fft_second_tw<A, -1, true>(v, twp);               // v[r] = C[2 (a + A r) + p]
+#else
         twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
@@ -235,6 +352,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
 #pragma unroll
             for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
         fft_second<A, -1>(v);                             // v[r] = C[2 (a + A r) + p]
+#endif
         // ---- split: rows k = 2 (a + A r) + p, r < 8, and k = n (thread a0, r = 8)
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -246,6 +364,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         }
         if (a0) stg_stream2(row(N), cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
     }
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -258,18 +377,39 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     extern __shared__ cplx ex[];
-    constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L, THREADS = R16Geom<A>::THREADS;
+    constexpr int N = R16Geom<A>::N, L = R16Geom<A>::L;
     const int tid = threadIdx.x, c = tid & 7, p = (tid >> 3) & 1, a = tid >> 4;
     const int nx = d.nx, ny = d.ny, y = blockIdx.y;
     const size_t x0 = (size_t)blockIdx.x * 2 * kCols;
     Ain += (size_t)blockIdx.z * (N + 1) * ny * nx;        // blockIdx.z: mesh of the batch
     phi += (size_t)blockIdx.z * N * ny * nx;
-    // all loads of the tile in flight at once (the last round is ragged: row k = N only)
-    constexpr int ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
     if (PDL) {
-        pdl_trigger();
+        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
+#if DKS_P5_DIRECT
+    // Every thread loads the 16 rows it needs itself, (FT{a}[r], FT{b}[r]) with one 256-bit load each, and forms its inputs
+    // C[K] in registers: C[K] = Fa[K] + i Fb[K] for K <= n, C[K] = conj Fa[L-K] + i conj Fb[L-K] above.  Row r serves K = r and
+    // K = L - r, i.e. two threads of the CTA: the second read is an L1 / L2 hit.  No pass through shared memory, no barrier.
+    cplx v[16];
+    {
+        const cplx *in0 = &Ain[(size_t)y * nx + x0 + 2 * c];
+#pragma unroll
+        for (int b = 0; b < 16; ++b) {
+            const int K = 2 * (a + A * b) + p;
+            const bool up = b >= 8 && K != N;                 // K > n: mirrored row, conjugated
+            cplx fa, fb;
+#if DKS_P5_LDCACHED
+            ldg_cached2(in0 + (size_t)(up ? L - K : K) * ny * nx, fa, fb);
+#else
+            ldg_stream2(in0 + (size_t)(up ? L - K : K) * ny * nx, fa, fb);
+#endif
+            v[b] = up ? cmake(fa.x + fb.y, fb.x - fa.y) : cmake(fa.x - fb.y, fa.y + fb.x);
+        }
+    }
+#else
+    // all loads of the tile in flight at once (the last round is ragged: row k = N only)
+    constexpr int THREADS = R16Geom<A>::THREADS, ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
     cplx fa[ROUNDS], fb[ROUNDS];
 #pragma unroll
     for (int i = 0; i < ROUNDS; ++i) {
@@ -292,9 +432,11 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ex[(2 * (a + A * b) + p) * kCols + c];
     __syncthreads();                                  // C consumed: ex becomes the exchange buffer
-    strided_inverse<A>(v, ex, c, p, a, tw1, tw2);
+#endif
+    strided_inverse<A, DKS_P5_TW_POST>(v, ex, c, p, a, tw1, tw2);
     cplx out[8];
     combine_parities<8>(v, p, out);
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
 #pragma unroll
     for (int i = 0; i < 8; ++i)
         stg_stream(reinterpret_cast<cplx *>(&phi[((size_t)(a + A * (i + 8 * p)) * ny + y) * nx + x0 + 2 * c]), out[i]);
@@ -357,7 +499,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * (16 * A) + p * P3Ex<A>::OFFP + j * P3Ex<A>::OFFJ;
     const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * GSTR;
     uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] group data, [1] Ghat rows
-    if (PDL) pdl_trigger();
+    if (PDL && !DKS_PDL_LATE) pdl_trigger();
     if (lane == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
@@ -475,6 +617,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             stg_stream(&base[a + A * (2 * i + p)], cadd(mine, shfl_xor_c(send, 1)));
         }
     }
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
 }
 
 }  // namespace dks

@@ -23,6 +23,10 @@
 #include "dks_greens_r16.cuh"
 #include "dks_field_ops.cuh"
 
+#ifndef DKS_PDL_MAX_NODES
+#define DKS_PDL_MAX_NODES (1 << 21)   // programmatic dependent launch for meshes of at most this many nodes
+#endif
+
 using namespace dks;
 
 // ------------------------------------------------------------------------------------------------
@@ -248,7 +252,7 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     p->smem_y = (size_t)2 * ny * p->Wy * sizeof(cplx);
     p->smem_z = (size_t)2 * nz * p->Wz * sizeof(cplx);
     p->slab = auto_slab(p);
-    p->pdl = (size_t)nx * ny * nz <= ((size_t)1 << 21);
+    p->pdl = (size_t)nx * ny * nz <= (size_t)DKS_PDL_MAX_NODES;
     compute_layout(p);
     g_err[0] = 0;
     return p;
