@@ -40,6 +40,9 @@ struct PeerTable {
 #ifndef DKS_TW_POST
 #define DKS_TW_POST 1
 #endif
+#ifndef DKS_P3_FOLD
+#define DKS_P3_FOLD 1
+#endif
 #ifndef DKS_P5_LDCACHED
 #define DKS_P5_LDCACHED 1
 #endif
@@ -164,6 +167,50 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
     strided_forward<A>(v, ex, c, p, a, tw1, tw2);
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
+#pragma unroll
+    for (int r = 0; r < 16; ++r)
+        stg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * r) + p) * nx + x], v[r]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// P2 with the two parities of a tile in two CTAs of 8 A threads each (blockIdx.x = 2 * tile + parity): the forward pass never
+// combines parities, so nothing is exchanged between them.  Parity-uniform CTAs issue the parity constants only where they are
+// used, and four CTAs of 128 threads per SM (instead of two of 256) overlap their load / transform / store phases more finely.
+// Both CTAs of a tile read the same rows: they are neighbours in launch order, so the second read is an L2 hit.
+// grid (2 nx / 8, planes)
+// ---------------------------------------------------------------------------------------------
+constexpr int kP2SplitMinA = 8;
+
+template <int A, bool PDL>
+__global__ void __launch_bounds__(8 * A, (DKS_R16_OCC / (8 * A) > 16 ? 16 : DKS_R16_OCC / (8 * A)))
+p2_y_fwd_r16p(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int kz0,
+              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
+{
+    extern __shared__ cplx ex[];                          // [16][A][8]
+    const int tid = threadIdx.x, c = tid & 7, a = tid >> 3, p = blockIdx.x & 1;
+    const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
+    const size_t x = (size_t)(blockIdx.x >> 1) * kCols + c;
+    if (PDL) {
+        if (!DKS_PDL_LATE) pdl_trigger();
+        pdl_wait();
+    }
+    cplx v[16];
+#pragma unroll
+    for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
+    if (p) parity_consts<-1>(v);
+    fft16<-1>(v);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) ex[(k * A + a) * kCols + c] = v[k];
+    cplx t[16];
+    load_tw_post<A>(t, tw1 + p * 16 * A, a);
+    __syncthreads();
+    constexpr int G = 16 / A;
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((a + A * g) * A + ap) * kCols + c];
+    fft_second_tw<A, -1, true>(v, t);
     if (PDL && DKS_PDL_LATE) pdl_trigger();
 #pragma unroll
     for (int r = 0; r < 16; ++r)
@@ -365,6 +412,58 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         if (a0) stg_stream2(row(N), cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
     }
     if (PDL && DKS_PDL_LATE) pdl_trigger();
+}
+
+// ---------------------------------------------------------------------------------------------
+// P1 with one CTA of 8 A threads per parity (blockIdx.x = 2 * tile + parity), loads straight to registers, not persistent.
+// The packed-spectrum split pairs C[k] with C[L-k], which have the same parity, so a parity's CTA splits and stores its own
+// rows; mirror partners sit 8 lanes apart (p1_a_of).  grid (2 nx / 16, ny, batch)
+// ---------------------------------------------------------------------------------------------
+template <int A, bool PDL>
+__global__ void __launch_bounds__(8 * A, (DKS_R16_OCC / (8 * A) > 16 ? 16 : DKS_R16_OCC / (8 * A)))
+p1_z_r2c_r16p(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d,
+              const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
+{
+    extern __shared__ cplx ex[];                          // [16][A][8]
+    constexpr int N = 16 * A;
+    const int tid = threadIdx.x, lane = tid & 31, c = tid & 7, p = blockIdx.x & 1;
+    const int a = p1_a_of<A>(p, (tid >> 3) & 1, tid >> 4);
+    const bool a0 = a == 0 && p == 0;
+    const int partner = (p == 0 && tid < 16) ? lane : lane ^ 8;
+    const int nx = d.nx, ny = d.ny, y = blockIdx.y;
+    const size_t xoff = (size_t)(blockIdx.x >> 1) * 2 * kCols + 2 * c;
+    rho += (size_t)blockIdx.z * N * ny * nx + (size_t)y * nx + xoff;
+    cplx *Aout = Aall + (size_t)blockIdx.z * (N + 1) * ny * nx + (size_t)y * nx + xoff;
+    if (PDL) {
+        if (!DKS_PDL_LATE) pdl_trigger();
+        pdl_wait();
+    }
+    cplx v[16];
+#pragma unroll
+    for (int b = 0; b < 16; ++b) v[b] = ldg_stream(reinterpret_cast<const cplx *>(&rho[(size_t)(a + A * b) * ny * nx]));
+    if (p) parity_consts<-1>(v);
+    fft16<-1>(v);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) ex[(k * A + a) * kCols + c] = v[k];
+    cplx t[16];
+    load_tw_post<A>(t, tw1 + p * 16 * A, a);
+    __syncthreads();
+    constexpr int G = 16 / A;
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((a + A * g) * A + ap) * kCols + c];
+    fft_second_tw<A, -1, true>(v, t);                     // v[r] = C[2 (a + A r) + p]
+    if (PDL && DKS_PDL_LATE) pdl_trigger();
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        cplx cm = cmake(__shfl_sync(0xffffffffu, v[15 - r].x, partner), __shfl_sync(0xffffffffu, v[15 - r].y, partner));
+        if (a0) cm = r == 0 ? v[0] : v[16 - r];
+        const cplx ck = v[r];
+        stg_stream2(Aout + (size_t)(2 * (a + A * r) + p) * ny * nx, cmake(0.5 * (ck.x + cm.x), 0.5 * (ck.y - cm.y)),
+                    cmake(0.5 * (ck.y + cm.y), -0.5 * (ck.x - cm.x)));
+    }
+    if (a0) stg_stream2(Aout + (size_t)N * ny * nx, cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -605,9 +704,13 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 #pragma unroll
             for (int k = 0; k < 16; ++k) v[k] = exw[k & 3][k * A];
         }
+#if DKS_P3_FOLD
+        fft16_tw<+1, false>(v, tb);                       // conj tb folded into the first butterfly layer (dks_fft_r16.cuh)
+#else
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = cmulc(v[k], tb[k]);
         fft16<+1>(v);
+#endif
         if (p) parity_consts<+1>(v);
         // combine the parities (crop fused): y[m] = O_0[m] + w_L^-m O_1[m]; parity 0 keeps the even registers, parity 1 the odd ones
 #pragma unroll

@@ -23,6 +23,12 @@
 #include "dks_greens_r16.cuh"
 #include "dks_field_ops.cuh"
 
+#ifndef DKS_P1_SPLIT
+#define DKS_P1_SPLIT 1
+#endif
+#ifndef DKS_P2_SPLIT
+#define DKS_P2_SPLIT 1
+#endif
 #ifndef DKS_PDL_MAX_NODES
 #define DKS_PDL_MAX_NODES (1 << 21)   // programmatic dependent launch for meshes of at most this many nodes
 #endif
@@ -311,6 +317,10 @@ static int r16_set_attributes()
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16p<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM / 2)); \
+    DKS_CUDA(cudaFuncSetAttribute(p1_z_r2c_r16p<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM / 2)); \
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16p<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM / 2)); \
+    DKS_CUDA(cudaFuncSetAttribute(p2_y_fwd_r16p<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM / 2)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p4_y_inv_r16<A_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
     DKS_CUDA(cudaFuncSetAttribute(p5_z_c2r_r16<A_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, R16Geom<A_>::SMEM)); \
@@ -353,11 +363,20 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
     const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
     switch (s.pass) {
     case 1: {
+        if (DKS_P1_SPLIT && A >= kP2SplitMinA) {
+            launch_pdl(p->pdl, p1_z_r2c_r16p<A, false>, p1_z_r2c_r16p<A, true>, dim3(2 * d.nx / (2 * kCols), d.ny, nb), dim3(T / 2), S / 2, st, rho, p->A, d, p->tw1[2], p->tw[2]);
+            break;
+        }
         const int tiles = d.nx / (2 * kCols) * d.ny * nb, per_sm = std::max(1, std::min(512 / T, (227 * 1024) / (P1Geom<A>::SMEM + 1024)));
         launch_pdl(p->pdl, p1_z_r2c_r16<A, false>, p1_z_r2c_r16<A, true>, dim3(std::min(tiles, p->sm_count * per_sm)), dim3(T), P1Geom<A>::SMEM, st, rho, p->A, d, nb, p->tw1[2], p->tw[2], PeerTable());
         break;
     }
-    case 2: launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]); break;
+    case 2:
+        if (DKS_P2_SPLIT && A >= kP2SplitMinA)    // one CTA per parity (CTAs of at least two warps)
+            launch_pdl(p->pdl, p2_y_fwd_r16p<A, false>, p2_y_fwd_r16p<A, true>, dim3(2 * d.nx / kCols, s.planes * nb), dim3(T / 2), S / 2, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]);
+        else
+            launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]);
+        break;
     case 4: launch_pdl(p->pdl, p4_y_inv_r16<A, false>, p4_y_inv_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->B, p->A, d, s.kz0, p->tw1[1], p->tw[1], PeerTable()); break;
     case 5: launch_pdl(p->pdl, p5_z_c2r_r16<A, false>, p5_z_c2r_r16<A, true>, dim3(d.nx / (2 * kCols), d.ny, nb), dim3(T), S, st, p->A, phi, d, p->tw1[2], p->tw[2]); break;
     }
