@@ -64,8 +64,11 @@ struct PeerTable {
 #ifndef DKS_P5_TW_POST
 #define DKS_P5_TW_POST true
 #endif
+// Programmatic dependent launch: the trigger sits right before a kernel's stores (late), not at its start.  An early trigger lets
+// the next kernel's CTAs take SM resources and spin in griddepcontrol.wait while this kernel still has CTAs to run
+// (measured: 64^3 31.2 -> 24.6 us per solve, 128^3 96.8 -> 92.7 us with the late trigger).
 #ifndef DKS_PDL_LATE
-#define DKS_PDL_LATE 0
+#define DKS_PDL_LATE 1
 #endif
 #ifndef DKS_R16_OCC
 #define DKS_R16_OCC 512

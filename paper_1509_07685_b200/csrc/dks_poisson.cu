@@ -222,9 +222,6 @@ extern "C" dks_poisson_plan *dks_poisson_plan_create(int nx, int ny, int nz, dou
     for (int a = 0; a < 3; ++a) {
         const int n = ns[a];
         if (n < 16 || n > 256) continue;
-        // meshes with every extent <= 16 stay on the tile kernels: five launches of a few CTAs each are launch-latency bound,
-        // and there the smaller kernels finish sooner (measured on B200: 16^3 at 36 k solves/s against 30 k)
-        if (nx <= 16 && ny <= 16 && nz <= 16) continue;
         const int A = n / 16, L = 2 * n;
         p->r16A[a] = A;
         // three regions of n entries (dks_fft_r16.cuh, twiddle_between): exp(-2 pi i e / L) with
