@@ -701,6 +701,9 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
                                     "p4_y_inv_generic", "p5_z_c2r_generic" };
     static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
     static const char *big_names[5] = { "p1_z_r2c_big", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_big" };
+    // P1 and P2 run one CTA per parity where a parity's CTA has at least two warps (launch_strided_r16)
+    if (pass == 1 && p->fast[0] && DKS_P1_SPLIT && p->r16A[2] >= kP2SplitMinA && p->nranks == 1) return "p1_z_r2c_r16p";
+    if (pass == 2 && p->fast[1] && DKS_P2_SPLIT && p->r16A[1] >= kP2SplitMinA) return "p2_y_fwd_r16p";
     return p->fast[pass - 1] ? fast_names[pass - 1] : p->big[pass - 1] ? big_names[pass - 1] : names[pass - 1];
 }
 

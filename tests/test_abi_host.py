@@ -123,6 +123,6 @@ def test_host_only_plan_options(dks):
     q = dks.dks_poisson_plan_create(128, 128, 128, 1e-4, 1e-4, 1e-4)
     try:
         assert [dks.dks_poisson_pass_name(q, i) for i in range(1, 6)] == [
-            "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"]
+            "p1_z_r2c_r16p", "p2_y_fwd_r16p", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"]   # n = 128: one CTA per parity
     finally:
         dks.dks_poisson_plan_destroy(q)

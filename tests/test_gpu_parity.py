@@ -506,7 +506,7 @@ def test_caller_owned_and_plan_owned_workspace(torch_cuda, dks, oracle, workload
 
 def test_long_line_passes_are_selected(dks):
     cases = {(64, 64, 512): ["p1_z_r2c_big", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_big"],
-             (512, 512, 256): ["p1_z_r2c_r16", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_r16"],
+             (512, 512, 256): ["p1_z_r2c_r16p", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_r16"],
              (8, 1024, 1024): ["p1_z_r2c_big", "p2_y_fwd_big", "p3_x_conv_generic", "p4_y_inv_big", "p5_z_c2r_big"],
              (16, 64, 16): ["p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"],
              (16, 16, 16): ["p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"],
