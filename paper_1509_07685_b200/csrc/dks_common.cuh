@@ -10,7 +10,6 @@ typedef double2 cplx;   // .x = re, .y = im
 __device__ __forceinline__ cplx cmake(double re, double im) { return make_double2(re, im); }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
 __device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
 // a * b
 __device__ __forceinline__ cplx cmul(cplx a, cplx b)
@@ -59,10 +58,10 @@ __device__ __forceinline__ void ldg_cached2(const cplx *p, cplx &v0, cplx &v1)
     asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v0.x), "=d"(v0.y), "=d"(v1.x), "=d"(v1.y) : "l"(p));
 }
 
-// Programmatic dependent launch (sm_90+).  Every pass kernel of the solve starts with pdl_trigger(): once all
-// CTAs of a grid have started, the next kernel in the stream may be scheduled into the SMs its tail frees
-// and run its prologue; pdl_wait() then blocks until the previous grid has completed and its memory is
-// visible.  Nothing the previous kernel wrote is read, and nothing it read is overwritten, before pdl_wait().
+// Programmatic dependent launch (sm_90+).  A PDL kernel calls pdl_trigger() right before its stores: once every CTA of the grid
+// has triggered or exited, the next kernel in the stream may be scheduled into the SMs the tail frees and run its prologue
+// (index arithmetic, twiddle loads, barrier initialisation); its pdl_wait() then blocks until the previous grid has completed
+// and its memory is visible.  Nothing the previous kernel wrote is read, and nothing it read is overwritten, before pdl_wait().
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
@@ -72,8 +71,6 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
     unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // ---- bulk asynchronous copy global -> shared (SASS UBLKCP) completing on an mbarrier -----------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }

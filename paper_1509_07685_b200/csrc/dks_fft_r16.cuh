@@ -227,14 +227,6 @@ __device__ __forceinline__ void twiddle_between(cplx (&v)[16], const cplx *__res
         v[k] = SIGN < 0 ? cmul(v[k], t) : cmulc(v[k], t);
     }
 }
-// same, table in shared memory
-template <int A, int SIGN>
-__device__ __forceinline__ void twiddle_between_s(cplx (&v)[16], const cplx *T, int a)
-{
-#pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = SIGN < 0 ? cmul(v[k], T[k * A + a]) : cmulc(v[k], T[k * A + a]);
-}
-
 // ---- twiddle AFTER the exchange ----------------------------------------------------------------
 // The between-step twiddle commutes with the exchange: the thread that holds sub-transform index k = a + A g after the
 // exchange multiplies its value from pre-exchange thread a' by T[k A + a'], i.e. by A consecutive table entries per g.

@@ -37,39 +37,12 @@ struct PeerTable {
     int first;               // P1: first global y row of this rank's slab;  P4: first global kz plane of this rank's slab
     int pitch;               // P1: global ny (rows per plane in the receiver);  P4: y rows per rank (rows per plane in the receiver)
 };
-#ifndef DKS_TW_POST
-#define DKS_TW_POST 1
-#endif
-#ifndef DKS_P3_FOLD
-#define DKS_P3_FOLD 1
-#endif
-#ifndef DKS_P5_LDCACHED
-#define DKS_P5_LDCACHED 1
-#endif
-#ifndef DKS_P5_DIRECT
-#define DKS_P5_DIRECT 1
-#endif
-#ifndef DKS_P1_BULK
-#define DKS_P1_BULK 1      // P1's stage completes on an mbarrier (no block barrier at the top of a tile)
-#endif
-#ifndef DKS_STAGE_BULK
-#define DKS_STAGE_BULK 0   // 1: one 128-byte cp.async.bulk per row instead of 16-byte cp.async (measured slower)
-#endif
-#if DKS_P1_BULK && !DKS_TW_POST
-#error DKS_P1_BULK needs DKS_TW_POST
-#endif
-#ifndef DKS_P4_TW_POST
-#define DKS_P4_TW_POST false
-#endif
-#ifndef DKS_P5_TW_POST
-#define DKS_P5_TW_POST true
-#endif
-// Programmatic dependent launch: the trigger sits right before a kernel's stores (late), not at its start.  An early trigger lets
-// the next kernel's CTAs take SM resources and spin in griddepcontrol.wait while this kernel still has CTAs to run
-// (measured: 64^3 31.2 -> 24.6 us per solve, 128^3 96.8 -> 92.7 us with the late trigger).
-#ifndef DKS_PDL_LATE
-#define DKS_PDL_LATE 1
-#endif
+// The between-step twiddle of an inverse strided pass is applied after the exchange in P5 and before it in P4 (measured:
+// P4, which runs at its memory bound, loses 2 % with the 16 table loads in flight across the barrier; P5 gains 1 %).
+constexpr bool kP4TwPost = false, kP5TwPost = true;
+// Programmatic dependent launch (PDL variants of the kernels): the trigger sits right before a kernel's stores, not at its start.
+// An early trigger lets the next kernel's CTAs take SM resources and spin in griddepcontrol.wait while this kernel still has CTAs
+// to run (measured: 64^3 31.2 -> 24.6 us per solve, 128^3 96.8 -> 92.7 us with the late trigger).
 #ifndef DKS_R16_OCC
 #define DKS_R16_OCC 512
 #endif
@@ -91,7 +64,6 @@ __device__ __forceinline__ void strided_forward(cplx (&v)[16], cplx *ex, int c, 
 {
     if (p) parity_consts<-1>(v);
     fft16<-1>(v);
-#if DKS_TW_POST
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
     cplx t[16];
@@ -103,18 +75,6 @@ __device__ __forceinline__ void strided_forward(cplx (&v)[16], cplx *ex, int c, 
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
     fft_second_tw<A, -1, true>(v, t);                    // regions 0 and 1 have T = 1 at a' = 0
-#else
-    twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
-#pragma unroll
-    for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
-    __syncthreads();
-    constexpr int G = 16 / A;
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-    fft_second<A, -1>(v);
-#endif
 }
 
 // inverse: v[b] = X[2 (a + A b) + p] on entry; on exit v[r] = IFFT_n(X_p)[a + A r] (* w_L^-(a + A r) if p)
@@ -123,30 +83,19 @@ __device__ __forceinline__ void strided_inverse(cplx (&v)[16], cplx *ex, int c, 
                                                 const cplx *__restrict__ tw1, const cplx *__restrict__ tw2)
 {
     fft16<+1>(v);
-    if (POST) {
-#pragma unroll
-    for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+    constexpr int G = 16 / A;
     cplx t[16];
-    load_tw_post<A>(t, tw1 + p * 32 * A, a);
-    __syncthreads();
-    constexpr int G = 16 / A;
-#pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-    fft_second_tw<A, +1, false>(v, t);                   // region 2 carries the thread constant w_L^(k mod A): no unit entry
-    } else {
-    twiddle_between<A, +1>(v, tw1 + p * 32 * A, a);
+    if (!POST) twiddle_between<A, +1>(v, tw1 + p * 32 * A, a);
 #pragma unroll
     for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
+    if (POST) load_tw_post<A>(t, tw1 + p * 32 * A, a);   // in flight across the barrier
     __syncthreads();
-    constexpr int G = 16 / A;
 #pragma unroll
     for (int g = 0; g < G; ++g)
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-    fft_second<A, +1>(v);
-    }
+    if (POST) fft_second_tw<A, +1, false>(v, t);         // region 2 carries the thread constant w_L^(k mod A): no unit entry
+    else fft_second<A, +1>(v);
     if (p) parity_consts<+1>(v);
 }
 
@@ -163,14 +112,13 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;          // kz: plane within the slab
     const size_t x = (size_t)blockIdx.x * kCols + c;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b) v[b] = ldg_stream(&Ain[((size_t)(kz0 + kz) * ny + a + A * b) * nx + x]);
     strided_forward<A>(v, ex, c, p, a, tw1, tw2);
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int r = 0; r < 16; ++r)
         stg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * r) + p) * nx + x], v[r]);
@@ -183,7 +131,7 @@ p2_y_fwd_r16(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, int
 // Both CTAs of a tile read the same rows: they are neighbours in launch order, so the second read is an L2 hit.
 // grid (2 nx / 8, planes)
 // ---------------------------------------------------------------------------------------------
-constexpr int kP2SplitMinA = 8;
+constexpr int kSplitMinA = 8;   // P1 and P2 run one CTA per parity for n >= 16 * kSplitMinA
 
 template <int A, bool PDL>
 __global__ void __launch_bounds__(8 * A, (DKS_R16_OCC / (8 * A) > 16 ? 16 : DKS_R16_OCC / (8 * A)))
@@ -195,7 +143,6 @@ p2_y_fwd_r16p(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, in
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
     const size_t x = (size_t)(blockIdx.x >> 1) * kCols + c;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
@@ -214,7 +161,7 @@ p2_y_fwd_r16p(const cplx *__restrict__ Ain, cplx *__restrict__ B, MeshDims d, in
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((a + A * g) * A + ap) * kCols + c];
     fft_second_tw<A, -1, true>(v, t);
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int r = 0; r < 16; ++r)
         stg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * r) + p) * nx + x], v[r]);
@@ -233,17 +180,16 @@ p4_y_inv_r16(const cplx *__restrict__ B, cplx *__restrict__ Aout, MeshDims d, in
     const int nx = d.nx, ny = d.ny, kz = blockIdx.y;
     const size_t x = (size_t)blockIdx.x * kCols + c;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
 #pragma unroll
     for (int b = 0; b < 16; ++b)
         v[b] = ldg_stream(&B[((size_t)kz * 2 * ny + 2 * (a + A * b) + p) * nx + x]);
-    strided_inverse<A, DKS_P4_TW_POST>(v, ex, c, p, a, tw1, tw2);
+    strided_inverse<A, kP4TwPost>(v, ex, c, p, a, tw1, tw2);
     cplx out[8];
     combine_parities<8>(v, p, out);
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int yrow = a + A * (i + 8 * p);
@@ -296,10 +242,9 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     const bool a0 = a == 0 && p == 0;                     // holds k = 0 and k = n, mirrors inside its own registers
     const int partner = (A == 1 || (p == 0 && tid < 32)) ? lane : lane ^ 16;
     const int nx = d.nx, ny = d.ny, xtiles = nx / (2 * kCols), tiles = xtiles * ny * nb;   // nb meshes back to back
-#if DKS_P1_BULK
     uint64_t *bar = reinterpret_cast<uint64_t *>(stage + N * kCols);      // [0] stage filled, [1] exchange buffer read
     if (tid == 0) {
-        mbar_init(&bar[0], DKS_STAGE_BULK ? 1 : THREADS);
+        mbar_init(&bar[0], THREADS);
         mbar_init(&bar[1], THREADS);
         mbar_init_fence();
     }
@@ -307,46 +252,20 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
     auto prefetch = [&](int t) {
         const int yy = t / xtiles, y = yy % ny;
         const double *src = rho + (size_t)(yy / ny) * N * ny * nx + (size_t)y * nx + (size_t)(t % xtiles) * 2 * kCols;
-#if DKS_STAGE_BULK
-        bulk_g2s(&stage[tid * kCols], &src[(size_t)tid * ny * nx], kCols * sizeof(cplx), &bar[0]);  // thread = input row z: 128 B
-#else
 #pragma unroll
         for (int i = 0; i < N * kCols / THREADS; ++i) {
             const int idx = tid + i * THREADS;
             cp_async16(&stage[idx], &src[(size_t)(idx >> 3) * ny * nx + 2 * (idx & 7)]);
         }
         cp_async_mbar_arrive(&bar[0]);
-#endif
     };
     unsigned phase = 0;
-#else
-    auto prefetch = [&](int t) {
-        const int yy = t / xtiles, y = yy % ny;
-        const double *src = rho + (size_t)(yy / ny) * N * ny * nx;
-        const size_t x0 = (size_t)(t % xtiles) * 2 * kCols;
-#pragma unroll
-        for (int i = 0; i < N * kCols / THREADS; ++i) {
-            const int idx = tid + i * THREADS, r = idx >> 3, cc = idx & 7;
-            cp_async16(&stage[idx], &src[((size_t)r * ny + y) * nx + x0 + 2 * cc]);
-        }
-        cp_async_commit();
-    };
-#endif
     int t = blockIdx.x;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();                                       // A is still being read by the previous solve's P5
     }
-#if DKS_P1_BULK
-    if (t < tiles) {
-        if (DKS_STAGE_BULK && tid == 0) mbar_expect_tx(&bar[0], N * kCols * sizeof(cplx));
-        prefetch(t);
-    }
-    for (; t < tiles; t += gridDim.x, phase ^= 1) {
-#else
     if (t < tiles) prefetch(t);
-    for (; t < tiles; t += gridDim.x) {
-#endif
+    for (; t < tiles; t += gridDim.x, phase ^= 1) {
         const int yy = t / xtiles, y = yy % ny;
         const size_t xoff = (size_t)(t % xtiles) * 2 * kCols + 2 * c;
         cplx *Aout = Aall + (size_t)(yy / ny) * (N + 1) * ny * nx + (size_t)y * nx + xoff;
@@ -356,29 +275,18 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
             const int o = min(k >> T.lsplit, T.nranks - 1);
             return T.base[o] + ((size_t)(k - (o << T.lsplit)) * T.pitch + T.first + y) * nx + xoff;
         };
-#if DKS_P1_BULK
         mbar_wait(&bar[0], phase);                        // stage complete
-#else
-        cp_async_wait_all();
-        __syncthreads();                                  // stage complete; last tile's exchange reads done
-#endif
         cplx v[16];
 #pragma unroll
         for (int b = 0; b < 16; ++b) v[b] = stage[(a + A * b) * kCols + c];
         // ---- strided_forward, with the prefetch of the next tile issued once the stage is consumed
         if (p) parity_consts<-1>(v);
         fft16<-1>(v);
-#if DKS_TW_POST
-#if DKS_P1_BULK
         if (t != (int)blockIdx.x) mbar_wait(&bar[1], phase ^ 1);          // the last tile's exchange reads are done
-#endif
 #pragma unroll
         for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
         cplx twp[16];
         load_tw_post<A>(twp, tw1 + p * 16 * A, a);
-#if DKS_P1_BULK
-        if (DKS_STAGE_BULK && tid == 0 && t + (int)gridDim.x < tiles) mbar_expect_tx(&bar[0], N * kCols * sizeof(cplx));
-#endif
         __syncthreads();
         if (t + (int)gridDim.x < tiles) prefetch(t + gridDim.x);
         constexpr int G = 16 / A;
@@ -386,23 +294,8 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         for (int g = 0; g < G; ++g)
 #pragma unroll
             for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-#if DKS_P1_BULK
         mbar_arrive(&bar[1]);
-#endif
         fft_second_tw<A, -1, true>(v, twp);               // v[r] = C[2 (a + A r) + p]
-#else
-        twiddle_between<A, -1>(v, tw1 + p * 16 * A, a);
-#pragma unroll
-        for (int k = 0; k < 16; ++k) ex[((p * 16 + k) * A + a) * kCols + c] = v[k];
-        __syncthreads();
-        if (t + (int)gridDim.x < tiles) prefetch(t + gridDim.x);
-        constexpr int G = 16 / A;
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((p * 16 + a + A * g) * A + ap) * kCols + c];
-        fft_second<A, -1>(v);                             // v[r] = C[2 (a + A r) + p]
-#endif
         // ---- split: rows k = 2 (a + A r) + p, r < 8, and k = n (thread a0, r = 8)
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -414,7 +307,7 @@ p1_z_r2c_r16(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims d
         }
         if (a0) stg_stream2(row(N), cmake(v[8].x, 0.0), cmake(v[8].y, 0.0));
     }
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -438,7 +331,6 @@ p1_z_r2c_r16p(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims 
     rho += (size_t)blockIdx.z * N * ny * nx + (size_t)y * nx + xoff;
     cplx *Aout = Aall + (size_t)blockIdx.z * (N + 1) * ny * nx + (size_t)y * nx + xoff;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
     cplx v[16];
@@ -457,7 +349,7 @@ p1_z_r2c_r16p(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims 
 #pragma unroll
         for (int ap = 0; ap < A; ++ap) v[g * A + ap] = ex[((a + A * g) * A + ap) * kCols + c];
     fft_second_tw<A, -1, true>(v, t);                     // v[r] = C[2 (a + A r) + p]
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         cplx cm = cmake(__shfl_sync(0xffffffffu, v[15 - r].x, partner), __shfl_sync(0xffffffffu, v[15 - r].y, partner));
@@ -486,10 +378,8 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
     Ain += (size_t)blockIdx.z * (N + 1) * ny * nx;        // blockIdx.z: mesh of the batch
     phi += (size_t)blockIdx.z * N * ny * nx;
     if (PDL) {
-        if (!DKS_PDL_LATE) pdl_trigger();
         pdl_wait();
     }
-#if DKS_P5_DIRECT
     // Every thread loads the 16 rows it needs itself, (FT{a}[r], FT{b}[r]) with one 256-bit load each, and forms its inputs
     // C[K] in registers: C[K] = Fa[K] + i Fb[K] for K <= n, C[K] = conj Fa[L-K] + i conj Fb[L-K] above.  Row r serves K = r and
     // K = L - r, i.e. two threads of the CTA: the second read is an L1 / L2 hit.  No pass through shared memory, no barrier.
@@ -501,44 +391,14 @@ p5_z_c2r_r16(const cplx *__restrict__ Ain, double *__restrict__ phi, MeshDims d,
             const int K = 2 * (a + A * b) + p;
             const bool up = b >= 8 && K != N;                 // K > n: mirrored row, conjugated
             cplx fa, fb;
-#if DKS_P5_LDCACHED
             ldg_cached2(in0 + (size_t)(up ? L - K : K) * ny * nx, fa, fb);
-#else
-            ldg_stream2(in0 + (size_t)(up ? L - K : K) * ny * nx, fa, fb);
-#endif
             v[b] = up ? cmake(fa.x + fb.y, fb.x - fa.y) : cmake(fa.x - fb.y, fa.y + fb.x);
         }
     }
-#else
-    // all loads of the tile in flight at once (the last round is ragged: row k = N only)
-    constexpr int THREADS = R16Geom<A>::THREADS, ITEMS = (N + 1) * kCols, ROUNDS = (ITEMS + THREADS - 1) / THREADS;
-    cplx fa[ROUNDS], fb[ROUNDS];
-#pragma unroll
-    for (int i = 0; i < ROUNDS; ++i) {
-        const int idx = tid + i * THREADS, k = idx >> 3, cc = idx & 7;
-        if (idx < ITEMS) {
-            const cplx *in = &Ain[((size_t)k * ny + y) * nx + x0 + 2 * cc];
-            ldg_stream2(in, fa[i], fb[i]);            // one 256-bit load: FT{a}[k], FT{b}[k] are neighbours
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < ROUNDS; ++i) {
-        const int idx = tid + i * THREADS, k = idx >> 3, cc = idx & 7;
-        if (idx < ITEMS) {
-            ex[k * kCols + cc] = cmake(fa[i].x - fb[i].y, fa[i].y + fb[i].x);
-            if (k > 0 && k < N) ex[(L - k) * kCols + cc] = cmake(fa[i].x + fb[i].y, fb[i].x - fa[i].y);
-        }
-    }
-    __syncthreads();
-    cplx v[16];
-#pragma unroll
-    for (int b = 0; b < 16; ++b) v[b] = ex[(2 * (a + A * b) + p) * kCols + c];
-    __syncthreads();                                  // C consumed: ex becomes the exchange buffer
-#endif
-    strided_inverse<A, DKS_P5_TW_POST>(v, ex, c, p, a, tw1, tw2);
+    strided_inverse<A, kP5TwPost>(v, ex, c, p, a, tw1, tw2);
     cplx out[8];
     combine_parities<8>(v, p, out);
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int i = 0; i < 8; ++i)
         stg_stream(reinterpret_cast<cplx *>(&phi[((size_t)(a + A * (i + 8 * p)) * ny + y) * nx + x0 + 2 * c]), out[i]);
@@ -601,7 +461,6 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     cplx *ex = reinterpret_cast<cplx *>(wb + kP3OffEx) + (j * 2 + p) * (16 * A) + p * P3Ex<A>::OFFP + j * P3Ex<A>::OFFJ;
     const double *gs = reinterpret_cast<const double *>(wb + kP3OffG) + j * GSTR;
     uint64_t *bar = reinterpret_cast<uint64_t *>(wb + kP3OffBar);     // [0] group data, [1] Ghat rows
-    if (PDL && !DKS_PDL_LATE) pdl_trigger();
     if (lane == 0) {
         mbar_init(&bar[0], 1);
         mbar_init(&bar[1], 1);
@@ -707,13 +566,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 #pragma unroll
             for (int k = 0; k < 16; ++k) v[k] = exw[k & 3][k * A];
         }
-#if DKS_P3_FOLD
         fft16_tw<+1, false>(v, tb);                       // conj tb folded into the first butterfly layer (dks_fft_r16.cuh)
-#else
-#pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = cmulc(v[k], tb[k]);
-        fft16<+1>(v);
-#endif
         if (p) parity_consts<+1>(v);
         // combine the parities (crop fused): y[m] = O_0[m] + w_L^-m O_1[m]; parity 0 keeps the even registers, parity 1 the odd ones
 #pragma unroll
@@ -723,7 +576,7 @@ p3_x_conv_r16(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
             stg_stream(&base[a + A * (2 * i + p)], cadd(mine, shfl_xor_c(send, 1)));
         }
     }
-    if (PDL && DKS_PDL_LATE) pdl_trigger();
+    if (PDL) pdl_trigger();
 }
 
 }  // namespace dks

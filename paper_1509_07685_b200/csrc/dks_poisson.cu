@@ -23,12 +23,6 @@
 #include "dks_greens_r16.cuh"
 #include "dks_field_ops.cuh"
 
-#ifndef DKS_P1_SPLIT
-#define DKS_P1_SPLIT 1
-#endif
-#ifndef DKS_P2_SPLIT
-#define DKS_P2_SPLIT 1
-#endif
 #ifndef DKS_PDL_MAX_NODES
 #define DKS_PDL_MAX_NODES (1 << 21)   // programmatic dependent launch for meshes of at most this many nodes
 #endif
@@ -360,7 +354,7 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
     const int T = R16Geom<A>::THREADS, S = R16Geom<A>::SMEM;
     switch (s.pass) {
     case 1: {
-        if (DKS_P1_SPLIT && A >= kP2SplitMinA) {
+        if (A >= kSplitMinA) {                          // one CTA per parity (CTAs of at least two warps)
             launch_pdl(p->pdl, p1_z_r2c_r16p<A, false>, p1_z_r2c_r16p<A, true>, dim3(2 * d.nx / (2 * kCols), d.ny, nb), dim3(T / 2), S / 2, st, rho, p->A, d, p->tw1[2], p->tw[2]);
             break;
         }
@@ -369,7 +363,7 @@ static void launch_strided_r16(const dks_poisson_plan::Step &s, const dks_poisso
         break;
     }
     case 2:
-        if (DKS_P2_SPLIT && A >= kP2SplitMinA)    // one CTA per parity (CTAs of at least two warps)
+        if (A >= kSplitMinA)
             launch_pdl(p->pdl, p2_y_fwd_r16p<A, false>, p2_y_fwd_r16p<A, true>, dim3(2 * d.nx / kCols, s.planes * nb), dim3(T / 2), S / 2, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]);
         else
             launch_pdl(p->pdl, p2_y_fwd_r16<A, false>, p2_y_fwd_r16<A, true>, dim3(d.nx / kCols, s.planes * nb), dim3(T), S, st, p->A, p->B, d, s.kz0, p->tw1[1], p->tw[1]);
@@ -702,8 +696,8 @@ extern "C" const char *dks_poisson_pass_name(const dks_poisson_plan *p, int pass
     static const char *fast_names[5] = { "p1_z_r2c_r16", "p2_y_fwd_r16", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16" };
     static const char *big_names[5] = { "p1_z_r2c_big", "p2_y_fwd_big", "p3_x_conv_big", "p4_y_inv_big", "p5_z_c2r_big" };
     // P1 and P2 run one CTA per parity where a parity's CTA has at least two warps (launch_strided_r16)
-    if (pass == 1 && p->fast[0] && DKS_P1_SPLIT && p->r16A[2] >= kP2SplitMinA && p->nranks == 1) return "p1_z_r2c_r16p";
-    if (pass == 2 && p->fast[1] && DKS_P2_SPLIT && p->r16A[1] >= kP2SplitMinA) return "p2_y_fwd_r16p";
+    if (pass == 1 && p->fast[0] && p->r16A[2] >= kSplitMinA && p->nranks == 1) return "p1_z_r2c_r16p";
+    if (pass == 2 && p->fast[1] && p->r16A[1] >= kSplitMinA) return "p2_y_fwd_r16p";
     return p->fast[pass - 1] ? fast_names[pass - 1] : p->big[pass - 1] ? big_names[pass - 1] : names[pass - 1];
 }
 
