@@ -95,7 +95,7 @@ int dks_poisson_solve_host(dks_poisson_plan *plan, const double *rho_host, doubl
 
 /* The same without the final synchronisation, so that consecutive steps overlap (PAPER.md:132 overlaps the rho
  * transfer with device work through streams): the copy-in of call i+1 and the copy-out of call i-1 run on
- * plan-owned streams beside the solve of call i, which runs on `stream`; two staging meshes alternate.  Every
+ * plan-owned streams beside the solve of call i, which runs on `stream`; three staging meshes take turns (a slot is busy from its copy-in to its copy-out).  Every
  * call still moves its own rho and phi.  phi_host of a call is complete after dks_poisson_host_sync (which
  * waits for every copy-out issued so far); rho_host must stay unchanged until then.  Pinned host memory is
  * needed for the overlap.  Not capturable in a CUDA graph. */
@@ -121,7 +121,7 @@ int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double
  * NaN restores the default rule G(r0), r0 = min(hx,hy,hz)/2.  Host-only.  Invalidates the Green's transform. */
 int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
 
-/* Bytes of device workspace the plan needs (buffer A, the Green's octant, the two host-path staging
+/* Bytes of device workspace the plan needs (buffer A, the Green's octant, the three host-path staging
  * meshes, one slab of B).  "Memory management is left up to the user": the caller may allocate it
  * (Fig. 2's allocateMemory) and attach it with dks_poisson_set_workspace.  Host-only. */
 size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);

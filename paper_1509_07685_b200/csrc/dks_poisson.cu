@@ -56,6 +56,11 @@ extern "C" const char *dks_last_error(void) { return g_err; }
 // ------------------------------------------------------------------------------------------------
 // plan
 // ------------------------------------------------------------------------------------------------
+// Staging meshes of the host path.  A slot is busy from the start of its copy-in to the end of its copy-out (the solve runs in place
+// on it): about 2.7 + 0.7 + 2.7 ms at 256^3 with both link directions busy.  Two slots allow one step per 3.05 ms; three make the
+// pipeline link-bound (one step per copy time, 2.7 ms).
+static const int kHostSlots = 3;
+
 struct dks_poisson_plan {
     MeshDims d;
     double hx, hy, hz;
@@ -78,10 +83,10 @@ struct dks_poisson_plan {
     size_t ws_bytes = 0;
     bool ws_owned = false;
     cplx *A = nullptr, *B = nullptr;
-    double *G = nullptr, *stage = nullptr;   // stage: two staging meshes (host path), back to back
+    double *G = nullptr, *stage = nullptr;   // stage: kHostSlots staging meshes (host path), back to back
     // host path pipeline (dks_poisson_solve_host_async): copy-in and copy-out streams and per-slot events
     cudaStream_t s_in = nullptr, s_out = nullptr;
-    cudaEvent_t ev_in[2] = { nullptr, nullptr }, ev_solve[2] = { nullptr, nullptr }, ev_out[2] = { nullptr, nullptr };
+    cudaEvent_t ev_in[kHostSlots] = {}, ev_solve[kHostSlots] = {}, ev_out[kHostSlots] = {};
     unsigned long long host_calls = 0;
     size_t offA, offB, offG, offS, need_bytes;
     // P2..P4 run slab by slab (slab = `slab` consecutive kz planes) so that B, the largest intermediate,
@@ -158,7 +163,7 @@ static void compute_layout(dks_poisson_plan *p)
         p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1) * nbm, 256);
     }
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
-    p->offS = off; off = align_up(off + 2 * align_up(8 * nx * ny * nz, 256), 256);
+    p->offS = off; off = align_up(off + kHostSlots * align_up(8 * nx * ny * nz, 256), 256);
     p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)(p->nranks > 1 ? p->planes_loc : p->slab) * nbm, 256);
     p->need_bytes = off;
     p->steps.clear();
@@ -274,7 +279,7 @@ static void release_device(dks_poisson_plan *p)
     p->setup_done = p->ghat_free = nullptr;
     if (p->s_setup) cudaStreamDestroy(p->s_setup);
     p->s_setup = nullptr;
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kHostSlots; ++i) {
         if (p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
         if (p->ev_solve[i]) cudaEventDestroy(p->ev_solve[i]);
         if (p->ev_out[i]) cudaEventDestroy(p->ev_out[i]);
@@ -833,7 +838,7 @@ extern "C" int dks_poisson_set_max_batch(dks_poisson_plan *p, int nbatch)
 
 // Host path.  Every call copies its rho to the device, solves and copies phi back, but consecutive calls
 // overlap: the copy-in of call i+1 and the copy-out of call i-1 run on their own streams beside the solve
-// of call i (PCIe is full duplex), as PAPER.md:132 does for the rho transfer.  Two staging meshes alternate.
+// of call i (PCIe is full duplex), as PAPER.md:132 does for the rho transfer.  kHostSlots staging meshes take turns.
 extern "C" int dks_poisson_solve_host_async(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
 {
     if (!p || !rho_host || !phi_host) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
@@ -842,16 +847,16 @@ extern "C" int dks_poisson_solve_host_async(dks_poisson_plan *p, const double *r
     if (!p->s_in) {
         DKS_CUDA(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking));
         DKS_CUDA(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < kHostSlots; ++i) {
             DKS_CUDA(cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming));
             DKS_CUDA(cudaEventCreateWithFlags(&p->ev_solve[i], cudaEventDisableTiming));
             DKS_CUDA(cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming));
         }
     }
     const size_t bytes = sizeof(double) * (size_t)p->d.nx * p->d.ny * p->d.nz;
-    const int slot = (int)(p->host_calls++ & 1);
+    const int slot = (int)(p->host_calls++ % kHostSlots);
     double *stage = p->stage + (size_t)slot * (align_up(bytes, 256) / sizeof(double));
-    if (p->host_calls > 2) DKS_CUDA(cudaStreamWaitEvent(p->s_in, p->ev_out[slot], 0));   // slot free again
+    if (p->host_calls > (unsigned long long)kHostSlots) DKS_CUDA(cudaStreamWaitEvent(p->s_in, p->ev_out[slot], 0));   // slot free again
     DKS_CUDA(cudaMemcpyAsync(stage, rho_host, bytes, cudaMemcpyHostToDevice, p->s_in));
     DKS_CUDA(cudaEventRecord(p->ev_in[slot], p->s_in));
     DKS_CUDA(cudaStreamWaitEvent(st, p->ev_in[slot], 0));

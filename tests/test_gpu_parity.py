@@ -434,7 +434,7 @@ def test_solve_host_path(torch_cuda, dks, oracle, workloads):
 
 
 def test_solve_host_async_pipeline(torch_cuda, dks, oracle, workloads):
-    # five pipelined steps with different inputs: every step's phi must be its own (two staging slots alternate)
+    # five pipelined steps with different inputs: every step's phi must be its own (three staging slots take turns)
     torch = torch_cuda
     n, h = (32, 16, 64), (2e-4, 3e-4, 1e-4)
     rhos = [workloads.random_rho(n, seed=40 + i) for i in range(5)]
