@@ -434,10 +434,11 @@ def test_solve_host_path(torch_cuda, dks, oracle, workloads):
 
 
 def test_solve_host_async_pipeline(torch_cuda, dks, oracle, workloads):
-    # five pipelined steps with different inputs: every step's phi must be its own (three staging slots take turns)
+    # eight pipelined steps with different inputs: every step's phi must be its own (three staging slots take turns, so every
+    # slot is reused at least twice and a copy-in has to wait for the copy-out that frees its slot)
     torch = torch_cuda
     n, h = (32, 16, 64), (2e-4, 3e-4, 1e-4)
-    rhos = [workloads.random_rho(n, seed=40 + i) for i in range(5)]
+    rhos = [workloads.random_rho(n, seed=40 + i) for i in range(8)]
     plan = dks.PoissonPlan(n, h)
     try:
         h_in = [torch.from_numpy(r).pin_memory() for r in rhos]
