@@ -189,6 +189,16 @@ int dks_gather_field(dks_poisson_plan *plan, const double *ex_dev, const double 
                      const double *x_dev, const double *y_dev, const double *z_dev, long long np, double ox, double oy, double oz,
                      double *epx_dev, double *epy_dev, double *epz_dev, void *stream);
 
+/* dks_gradient followed by dks_gather_field in one call, for the per-step use: the field at the particles
+ * straight from phi, readings F3 + F4, same results as the two calls.  The node field is not returned; it lives for the duration
+ * of the call in the plan's buffer B, interleaved (ex, ey, ez per node in one 32-byte record, so the gather needs one 256-bit load
+ * per node).  Needs the plan's workspace (dks_poisson_set_workspace or a previous dks_greens_setup; DKS_ERR_NOT_SETUP otherwise)
+ * and the unslabbed, unsharded pipeline (DKS_ERR_INVALID_ARG otherwise); must not run concurrently with a solve of the same
+ * plan (both use B).  Asynchronous on `stream`. */
+int dks_field_at_particles(dks_poisson_plan *plan, const double *phi_dev, const double *x_dev, const double *y_dev,
+                           const double *z_dev, long long np, double ox, double oy, double oz, double *epx_dev, double *epy_dev,
+                           double *epz_dev, void *stream);
+
 /* ---- One solve sharded over several GPUs (SURVEY.md sections 8(e), 8(f3)) ------------------------------------------------
  * The paper never splits a solve: several MPI ranks share ONE GPU through CUDA IPC.  This is the
  * contrasting B200 design: rank r of g (g a power of two <= 8; nx, ny, nz in [32, 256]) owns the y rows

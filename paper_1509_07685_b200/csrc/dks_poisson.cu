@@ -964,6 +964,29 @@ extern "C" int dks_gather_field(dks_poisson_plan *p, const double *ex, const dou
     return DKS_OK;
 }
 
+// dks_gradient followed by dks_gather_field without the three field meshes: the field lives for the duration of the call in the
+// plan's buffer B (free between solves), interleaved (dks_field_ops.cuh).
+extern "C" int dks_field_at_particles(dks_poisson_plan *p, const double *phi, const double *x, const double *y, const double *z,
+                                      long long np, double ox, double oy, double oz, double *epx, double *epy, double *epz, void *stream)
+{
+    if (!p || !phi || np < 0 || (np > 0 && (!x || !y || !z || !epx || !epy || !epz)))
+        return fail(DKS_ERR_INVALID_ARG, "plan, phi or a particle array is NULL, or np < 0");
+    if (!std::isfinite(ox) || !std::isfinite(oy) || !std::isfinite(oz)) return fail(DKS_ERR_INVALID_ARG, "origin must be finite");
+    if (!p->ws || !p->B) return fail(DKS_ERR_NOT_SETUP, "dks_field_at_particles uses the plan's workspace: attach one or call dks_greens_setup first");
+    if (p->nranks > 1 || p->slab != p->d.nz + 1)
+        return fail(DKS_ERR_INVALID_ARG, "dks_field_at_particles needs the full buffer B: not available on slabbed or sharded plans");
+    int rc = ensure_device(p);
+    if (rc) return rc;
+    if (np == 0) return DKS_OK;
+    const MeshDims d = p->d;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    double4 *e = reinterpret_cast<double4 *>(p->B);            // 32 nx ny nz bytes <= 32 nx ny (nz + 1) = sizeof B
+    gradient_aos_kernel<<<dim3((d.nx + 127) / 128, d.ny, d.nz), 128, 0, st>>>(phi, e, d, 0.5 / p->hx, 0.5 / p->hy, 0.5 / p->hz);
+    gather_aos_kernel<<<particle_grid(p, np), 256, 0, st>>>(e, x, y, z, np, frame_of(p, ox, oy, oz), d, epx, epy, epz);
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // f3: one solve sharded over several GPUs; DESIGN.md section 9
 // ------------------------------------------------------------------------------------------------

@@ -49,6 +49,7 @@ SYMBOLS = {
     "dks_deposit_cic": (_i, [_vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp]),
     "dks_gradient": (_i, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dks_gather_field": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
+    "dks_field_at_particles": (_i, [_vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "dks_poisson_set_shard": (_i, [_vp, _i, _i]),
     "dks_poisson_shard_buffers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
     "dks_poisson_set_peers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
@@ -215,6 +216,11 @@ def dks_gather_field(plan, ex, ey, ez, x, y, z, np_, origin, epx, epy, epz, stre
                                        *(float(v) for v in origin), _ptr(epx), _ptr(epy), _ptr(epz), stream), "dks_gather_field")
 
 
+def dks_field_at_particles(plan, phi, x, y, z, np_, origin, epx, epy, epz, stream=None):
+    return _check(lib.dks_field_at_particles(plan, _ptr(phi), _ptr(x), _ptr(y), _ptr(z), int(np_), *(float(v) for v in origin),
+                                             _ptr(epx), _ptr(epy), _ptr(epz), stream), "dks_field_at_particles")
+
+
 def dks_poisson_set_shard(plan, rank, nranks):
     return _check(lib.dks_poisson_set_shard(plan, int(rank), int(nranks)), "dks_poisson_set_shard")
 
@@ -345,6 +351,13 @@ class PoissonPlan:
 
         epx, epy, epz = torch.empty_like(x), torch.empty_like(x), torch.empty_like(x)
         dks_gather_field(self._plan, ex, ey, ez, x, y, z, x.numel(), origin, epx, epy, epz, torch.cuda.current_stream().cuda_stream)
+        return epx, epy, epz
+
+    def field_at_particles(self, phi, x, y, z, origin):
+        import torch
+
+        epx, epy, epz = torch.empty_like(x), torch.empty_like(x), torch.empty_like(x)
+        dks_field_at_particles(self._plan, phi, x, y, z, x.numel(), origin, epx, epy, epz, torch.cuda.current_stream().cuda_stream)
         return epx, epy, epz
 
     def greens_hat(self):

@@ -86,6 +86,18 @@ def test_deposit_degenerate(torch_cuda, dks):
             dks.dks_deposit_cic(plan.handle, far, far, far, far, -1, (0, 0, 0), rho, None)
         with pytest.raises(dks.DksError):
             dks.dks_gradient(plan.handle, rho, rho, rho, rho, None)                                  # outputs alias phi
+        with pytest.raises(dks.DksError):
+            dks.dks_field_at_particles(plan.handle, rho, far, far, far, -1, (0, 0, 0), far, far, far, None)
+        out = [torch.full((5,), 3.0, dtype=torch.float64, device="cuda") for _ in range(3)]
+        dks.dks_field_at_particles(plan.handle, rho, far, far, far, 5, (0.0, 0.0, 0.0), *out, None)  # all dropped: field 0
+        assert all(float(o.abs().max()) == 0.0 for o in out)
+        bare = dks.dks_poisson_plan_create(8, 16, 8, 1e-3, 1e-3, 1e-3)                                # no workspace yet
+        try:
+            with pytest.raises(dks.DksError) as e:
+                dks.dks_field_at_particles(bare, rho, far, far, far, 5, (0, 0, 0), *out, None)
+            assert e.value.status == dks.DKS_ERR_NOT_SETUP
+        finally:
+            dks.dks_poisson_plan_destroy(bare)
     finally:
         plan.close()
 
@@ -106,10 +118,12 @@ def test_gradient_and_gather(torch_cuda, dks, oracle, workloads, n, h):
         for got, ref in ((ex, rex), (ey, rey), (ez, rez)):
             assert np.max(np.abs(got.cpu().numpy() - ref)) <= bound
         epx, epy, epz = plan.gather(ex, ey, ez, dx, dy, dz, origin)
-        for got, field in ((epx, rex), (epy, rey), (epz, rez)):
+        fused = plan.field_at_particles(d_phi, dx, dy, dz, origin)         # the same two steps in one call, interleaved scratch
+        for got, got_fused, field in ((epx, fused[0], rex), (epy, fused[1], rey), (epz, fused[2], rez)):
             ref = oracle.cic_gather(field, n, h, origin, x, y, z)
-            assert np.max(np.abs(got.cpu().numpy() - ref)) <= 1e-14 * np.max(np.abs(field)) + bound
-            assert np.count_nonzero(ref == 0.0) > 0 and np.array_equal(got.cpu().numpy() == 0.0, ref == 0.0)   # dropped particles
+            for g in (got, got_fused):
+                assert np.max(np.abs(g.cpu().numpy() - ref)) <= 1e-14 * np.max(np.abs(field)) + bound
+                assert np.count_nonzero(ref == 0.0) > 0 and np.array_equal(g.cpu().numpy() == 0.0, ref == 0.0)   # dropped particles
     finally:
         plan.close()
 
@@ -127,8 +141,7 @@ def test_space_charge_step_on_device_matches_oracle_chain(torch_cuda, dks, oracl
         dx, dy, dz, dq = dev(torch, x, y, z, q)
         rho = plan.deposit(dx, dy, dz, dq, origin)
         phi = plan.solve(rho)
-        ex, ey, ez = plan.gradient(phi)
-        ep = plan.gather(ex, ey, ez, dx, dy, dz, origin)
+        ep = plan.field_at_particles(phi, dx, dy, dz, origin)
         got_phi = phi.cpu().numpy()
         assert np.linalg.norm((got_phi - phi_ref).ravel()) <= 1e-12 * np.linalg.norm(phi_ref.ravel())
         emax = max(np.max(np.abs(c)) for c in e_ref)
