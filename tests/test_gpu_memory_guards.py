@@ -24,6 +24,7 @@ def guards_intact(torch, buf, numel):
 
 
 SHAPES = [(8, 8, 8), (16, 8, 32), (16, 16, 64), (32, 16, 64), (64, 64, 16), (128, 32, 16), (256, 16, 8), (16, 256, 32), (8, 32, 256),
+          (16, 16, 128), (32, 128, 256),           # per-parity P1 / P2 kernels (n >= 128 on z / y)
           (512, 8, 16), (8, 8, 1024), (16, 512, 8)]
 
 

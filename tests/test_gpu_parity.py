@@ -148,7 +148,8 @@ def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
 
 # ---- batched solves: several meshes per launch, one Green's transform ------------------------------------
 @pytest.mark.parametrize("n,h", [((32, 16, 64), (2e-4, 3e-4, 1e-4)), ((64, 64, 64), (5e-4, 5e-4, 5e-4)),
-                                 ((8, 16, 8), (1e-3, 1e-3, 2e-3)), ((128, 32, 16), (1e-4, 2e-4, 4e-4))])
+                                 ((8, 16, 8), (1e-3, 1e-3, 2e-3)), ((128, 32, 16), (1e-4, 2e-4, 4e-4)),
+                                 ((32, 128, 128), (2e-4, 1e-4, 3e-4))])                      # per-parity P1 and P2 kernels
 def test_solve_batch_matches_single_solves_and_oracle(torch_cuda, dks, oracle, workloads, n, h):
     torch = torch_cuda
     nb = 3
