@@ -37,7 +37,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (default 4 = 256^3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--e2e-steps", type=int, default=60, help="host-path steps per e2e loop (pipeline fill and drain are inside the timed region)")
     ap.add_argument("--slab", type=int, default=None, help="planes per P2-P4 slab (default: the plan's automatic choice)")
     ap.add_argument("--prof-steps", type=int, default=50, help="extra solves with per-launch events, for the per-pass split")
     ap.add_argument("--no-cpu-baseline", action="store_true")
