@@ -41,6 +41,7 @@ def parse():
     ap.add_argument("--slab", type=int, default=None, help="planes per P2-P4 slab (default: the plan's automatic choice)")
     ap.add_argument("--prof-steps", type=int, default=50, help="extra solves with per-launch events, for the per-pass split")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the torch.fft (cuFFT) side reference")
     ap.add_argument("--ref-sample", action="store_true",
                     help="--impl reference: time the central half-extent sub-mesh instead of the full mesh (reported unscaled, under its own workload name)")
     ap.add_argument("--repeats", type=int, default=5, help="timed windows of --steps solves each; the median is reported")
@@ -206,6 +207,41 @@ def run_reference(args):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def cufft_side_reference(torch, w, d_rho, d_phi, stream, reps=10):
+    """Padded rfftn -> multiply by the complex half-spectrum of G -> irfftn -> crop with torch.fft (cuFFT), Green's transform
+    precomputed; d_phi (the product's result for d_rho) is only used to check that the side reference computes the same thing."""
+    import math
+    nx, ny, nz = w.n
+    hx, hy, hz = w.h
+    k = 1.0 / (4.0 * math.pi * 8.8541878128e-12)
+
+    def mirrored(n, h):
+        i = torch.arange(2 * n, device="cuda", dtype=torch.float64)
+        return torch.minimum(i, 2 * n - i) * h
+
+    r = torch.sqrt(mirrored(nz, hz)[:, None, None] ** 2 + mirrored(ny, hy)[None, :, None] ** 2 + mirrored(nx, hx)[None, None, :] ** 2)
+    r[0, 0, 0] = 0.5 * min(hx, hy, hz)
+    ghat = torch.fft.rfftn(k / r) * (hx * hy * hz)
+    del r
+    shape = (2 * nz, 2 * ny, 2 * nx)
+
+    def solve():
+        return torch.fft.irfftn(torch.fft.rfftn(d_rho, s=shape) * ghat, s=shape)[:nz, :ny, :nx]
+
+    out = solve()
+    rel = float(torch.linalg.norm((out - d_phi).flatten()) / torch.linalg.norm(d_phi.flatten()))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        out = solve()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    return {"value": 1e3 / ms, "unit": UNIT, "ms_per_step": ms, "rel_l2_vs_product": rel,
+            "what": "torch.fft.rfftn(rho, s = doubled grid) * FT{G} -> irfftn -> crop (cuFFT, fp64), FT{G} precomputed; "
+                    "the pipeline of PAPER.md:132 on this GPU, context only"}
 
 
 def run_ours(args):
@@ -444,6 +480,16 @@ def run_ours(args):
     }
     plan.close()
 
+    # ---- side reference (north_star: "cuFFT may be timed as a side reference"): the paper-style pipeline
+    # of PAPER.md:132 -- library FFT of the zero-padded mesh, separate multiplication, library inverse FFT, crop -- through
+    # torch.fft (cuFFT) on the same GPU, Green's transform precomputed as for the product.  Context only: no product code.
+    cufft = None
+    if world == 1 and not args.no_cufft:
+        try:
+            cufft = cufft_side_reference(torch, w, d_rho, d_phi, stream)
+        except Exception as e:                          # e.g. out of memory on a smaller device: the side reference is optional
+            cufft = {"unavailable": repr(e)[:200]}
+
     # ---- CPU oracle timed beside it (rank 0, N = 1 only) ---------------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -479,6 +525,8 @@ def run_ours(args):
         "gpu_launches": launches * args.steps,
         "roofline": roofline,
     }
+    if cufft is not None:
+        line["cufft_side_reference"] = cufft
     if cpu is not None:
         line["cpu_baseline"] = cpu
     print(json.dumps(line), flush=True)

@@ -146,6 +146,32 @@ def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
     assert np.max(np.abs(g - direct) / np.abs(direct)) <= 1e-11
 
 
+def test_full_size_agreement_with_a_library_fft_on_the_gpu(torch_cuda, dks, workloads):
+    # A third opinion at a size the long-double oracle needs minutes for: the same convolution through torch.fft (cuFFT) on the doubled
+    # grid of config 3 (the library special case of pin P12, run on the GPU).  Not the oracle: an independent FFT, same readings A1-A5.
+    torch = torch_cuda
+    w = workloads.config(3)
+    (nx, ny, nz), (hx, hy, hz) = w.n, w.h
+    d_rho = torch.from_numpy(workloads.make_rho(w)).cuda()
+
+    def mirrored(n, h):
+        i = torch.arange(2 * n, device="cuda", dtype=torch.float64)
+        return torch.minimum(i, 2 * n - i) * h
+
+    r = torch.sqrt(mirrored(nz, hz)[:, None, None] ** 2 + mirrored(ny, hy)[None, :, None] ** 2 + mirrored(nx, hx)[None, None, :] ** 2)
+    r[0, 0, 0] = 0.5 * min(hx, hy, hz)
+    g = 1.0 / (4.0 * np.pi * 8.8541878128e-12 * r)
+    shape = (2 * nz, 2 * ny, 2 * nx)
+    ref = torch.fft.irfftn(torch.fft.rfftn(d_rho, s=shape) * torch.fft.rfftn(g), s=shape)[:nz, :ny, :nx] * (hx * hy * hz)
+    plan = dks.PoissonPlan(w.n, w.h)
+    try:
+        got = plan.solve(d_rho)
+        assert float(torch.linalg.norm((got - ref).flatten()) / torch.linalg.norm(ref.flatten())) <= REL_L2_TOL
+        assert float((got - ref).abs().max()) <= MAX_ABS_TOL * float(ref.abs().max())
+    finally:
+        plan.close()
+
+
 # ---- batched solves: several meshes per launch, one Green's transform ------------------------------------
 @pytest.mark.parametrize("n,h", [((32, 16, 64), (2e-4, 3e-4, 1e-4)), ((64, 64, 64), (5e-4, 5e-4, 5e-4)),
                                  ((8, 16, 8), (1e-3, 1e-3, 2e-3)), ((128, 32, 16), (1e-4, 2e-4, 4e-4)),
