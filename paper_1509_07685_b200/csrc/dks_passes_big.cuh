@@ -12,7 +12,7 @@
 namespace dks {
 
 // ---- P2: forward y.  grid (nx / W, planes * batch) ---------------------------------------------------------------------
-template <int L>
+template <int L, bool PDL = false>
 __global__ void __launch_bounds__(BigGeom<L>::THREADS, BigGeom<L>::MINB)
 p2_y_fwd_big(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, int kz0, const cplx *__restrict__ tw)
 {
@@ -25,6 +25,7 @@ p2_y_fwd_big(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, int k
     const cplx *in = A + ((size_t)(kz0 + blockIdx.y) * N) * nx + x;
     cplx *out = B + ((size_t)blockIdx.y * L) * nx + x;
     cplx v[16];
+    if (PDL) pdl_wait();
 #pragma unroll
     for (int m = 0; m < 16; ++m) v[m] = m < 8 ? ldg_stream(&in[(size_t)(u + G::S1 * m) * nx]) : cmake(0.0, 0.0);
     St::fwd1(v, tw, u);
@@ -34,12 +35,13 @@ p2_y_fwd_big(const cplx *__restrict__ A, cplx *__restrict__ B, MeshDims d, int k
     __syncthreads();
     St::get3(s, v, u, w);
     St::template bfly3<-1>(v);
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int i = 0; i < 16; ++i) stg_stream(&out[(size_t)big_freq_of<L>(16 * u + i) * nx], v[i]);
 }
 
 // ---- P4: inverse y, crop -----------------------------------------------------------------------------------------------
-template <int L>
+template <int L, bool PDL = false>
 __global__ void __launch_bounds__(BigGeom<L>::THREADS, BigGeom<L>::MINB)
 p4_y_inv_big(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, int kz0, const cplx *__restrict__ tw)
 {
@@ -52,6 +54,7 @@ p4_y_inv_big(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, int k
     const cplx *in = B + ((size_t)blockIdx.y * L) * nx + x;
     cplx *out = A + ((size_t)(kz0 + blockIdx.y) * N) * nx + x;
     cplx v[16];
+    if (PDL) pdl_wait();
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = ldg_stream(&in[(size_t)big_freq_of<L>(16 * u + i) * nx]);
     St::template bfly3<+1>(v);
@@ -61,12 +64,13 @@ p4_y_inv_big(const cplx *__restrict__ B, cplx *__restrict__ A, MeshDims d, int k
     __syncthreads();
     St::get1(s, v, u, w);
     St::inv1(v, tw, u);
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int q = 0; q < 8; ++q) stg_stream(&out[(size_t)(u + G::S1 * q) * nx], v[q]);
 }
 
 // ---- P1: forward z, real -> complex (two real columns packed into one complex line, split afterwards) -----------------
-template <int L>
+template <int L, bool PDL = false>
 __global__ void __launch_bounds__(BigGeom<L>::THREADS, BigGeom<L>::MINB)
 p1_z_r2c_big(const double *__restrict__ rho, cplx *__restrict__ A, MeshDims d, const cplx *__restrict__ tw)
 {
@@ -78,6 +82,7 @@ p1_z_r2c_big(const double *__restrict__ rho, cplx *__restrict__ A, MeshDims d, c
     rho += (size_t)blockIdx.z * N * ny * nx;              // blockIdx.z: mesh of the batch
     A += (size_t)blockIdx.z * (N + 1) * ny * nx;
     cplx v[16];
+    if (PDL) pdl_wait();                                  // A is still being read by the previous solve's P5
 #pragma unroll
     for (int m = 0; m < 16; ++m)
         v[m] = m < 8 ? ldg_stream(reinterpret_cast<const cplx *>(&rho[((size_t)(u + G::S1 * m) * ny + y) * nx + x0 + 2 * w])) : cmake(0.0, 0.0);
@@ -90,6 +95,7 @@ p1_z_r2c_big(const double *__restrict__ rho, cplx *__restrict__ A, MeshDims d, c
     St::template bfly3<-1>(v);
     St::put3(s, v, u, w);
     __syncthreads();
+    if (PDL) pdl_trigger();
     for (int idx = tid; idx < (N + 1) * W; idx += NT) {
         const int k = idx / W, ww = idx % W;
         const cplx ck = s[big_pos_of<L>(k) * W + ww], cm = s[big_pos_of<L>((L - k) & (L - 1)) * W + ww];
@@ -99,7 +105,7 @@ p1_z_r2c_big(const double *__restrict__ rho, cplx *__restrict__ A, MeshDims d, c
 }
 
 // ---- P5: inverse z, complex -> real, crop ------------------------------------------------------------------------------
-template <int L>
+template <int L, bool PDL = false>
 __global__ void __launch_bounds__(BigGeom<L>::THREADS, BigGeom<L>::MINB)
 p5_z_c2r_big(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims d, const cplx *__restrict__ tw)
 {
@@ -110,6 +116,7 @@ p5_z_c2r_big(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims d, c
     const int nx = d.nx, ny = d.ny, x0 = blockIdx.x * 2 * W, y = blockIdx.y, tid = threadIdx.x, w = tid % W, u = tid / W;
     A += (size_t)blockIdx.z * (N + 1) * ny * nx;
     phi += (size_t)blockIdx.z * N * ny * nx;
+    if (PDL) pdl_wait();
 #pragma unroll 2
     for (int idx = tid; idx < (N + 1) * W; idx += NT) {
         const int k = idx / W, ww = idx % W;
@@ -129,6 +136,7 @@ p5_z_c2r_big(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims d, c
     __syncthreads();
     St::get1(s, v, u, w);
     St::inv1(v, tw, u);
+    if (PDL) pdl_trigger();
 #pragma unroll
     for (int q = 0; q < 8; ++q)
         stg_stream(reinterpret_cast<cplx *>(&phi[((size_t)(u + G::S1 * q) * ny + y) * nx + x0 + 2 * w]), v[q]);
@@ -143,7 +151,7 @@ struct P3BigGeom {
     static constexpr int SMEM = BigGeom<L>::SMEMX + BigGeom<L>::W * GROW * (int)sizeof(double);
 };
 
-template <int L>
+template <int L, bool PDL = false>
 __global__ void __launch_bounds__(BigGeom<L>::THREADS, 1)
 p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, const cplx *__restrict__ tw)
 {
@@ -156,6 +164,7 @@ p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     const int line0 = blockIdx.x * W;
     const int kz = (kz0 + line0 / (2 * ny)) % (d.nz + 1), ky0 = line0 % (2 * ny);    // a batch repeats kz
     cplx *base = B + (size_t)line0 * N;
+    if (PDL) pdl_wait();
 #pragma unroll 4
     for (int idx = tid; idx < N * W; idx += NT) {
         const int ww = idx / N, pp = idx % N;
@@ -192,6 +201,7 @@ p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     __syncthreads();                                      // all stage-1 reads done before the cropped result is written
     St::put1(s, v, u, w, 8);
     __syncthreads();
+    if (PDL) pdl_trigger();
 #pragma unroll 4
     for (int idx = tid; idx < N * W; idx += NT) {
         const int ww = idx / N, pp = idx % N;
