@@ -362,8 +362,8 @@ p1_z_r2c_r16p(const double *__restrict__ rho, cplx *__restrict__ Aall, MeshDims 
 }
 
 // ---------------------------------------------------------------------------------------------
-// P5: inverse z, complex -> real, crop to nz.  Rebuilds the packed spectrum C[k] = Fa[k] + i Fb[k],
-// C[L-k] = conj Fa[k] + i conj Fb[k] in shared memory first.  grid (nx / 16, ny)
+// P5: inverse z, complex -> real, crop to nz.  The inverse of P1's split: the packed spectrum C[k] = Fa[k] + i Fb[k],
+// C[L-k] = conj Fa[k] + i conj Fb[k] is formed in registers from the rows each thread loads itself.  grid (nx / 16, ny, batch)
 // ---------------------------------------------------------------------------------------------
 template <int A, bool PDL>
 __global__ void __launch_bounds__(R16Geom<A>::THREADS, DKS_R16_MINB(A))
