@@ -199,6 +199,34 @@ int dks_field_at_particles(dks_poisson_plan *plan, const double *phi_dev, const 
                            const double *z_dev, long long np, double ox, double oy, double oz, double *epx_dev, double *epy_dev,
                            double *epz_dev, void *stream);
 
+/* ---- The field at the particles without any device allocation ---------------------------------------------------------------
+ * Same operation and same results as dks_field_at_particles (gradient of phi by second-order differences, readings F3 + F4,
+ * then trilinear interpolation to the particles), for callers that cannot allocate device memory: no plan
+ * is needed (creating and using a plan calls cudaMalloc for its tables and, unless one is attached, its workspace).  Who
+ * that is: a time-step loop whose other streams a cudaMalloc / cudaFree would stall, because both synchronise the device; a
+ * host program whose own pool already holds all device memory, so that any further cudaMalloc fails; a component that is
+ * only ever handed device pointers and has no allocator of its own.
+ *
+ * The node field (one 32-byte record per node) goes into an array that is part of the library image: 8 MiB of device
+ * memory, held by every GPU on which the library's CUDA module is loaded until the process exits.  Hence the limit
+ * nx * ny * nz <= DKS_STATIC_FIELD_MAX_NODES (64 x 64 x 64, 128 x 64 x 32, ...); a larger mesh is refused with
+ * DKS_ERR_INVALID_ARG and a message naming the limit.  nx, ny, nz: powers of two in [8, 1024] as for a plan; hx, hy, hz > 0.
+ * phi_dev [nz][ny][nx], the particle arrays (np entries each) and the three outputs are DEVICE pointers the caller owns;
+ * the call itself never calls cudaMalloc, cudaFree or any library routine that allocates.
+ *
+ * First call on a device: looks up the device address of the array (cudaGetSymbolAddress, with that device current) and the
+ * SM count, and keeps them for later calls.  Make that first call outside any stream capture.  Later calls only launch two
+ * kernels on `stream` (asynchronous, no synchronisation).
+ *
+ * All calls on one device share the one array.  It keeps whatever the last call wrote; that is harmless, because a call
+ * writes the record of every node of its mesh before it reads any.  But two calls that are in flight on the same GPU at
+ * the same time (different streams, or different host threads) overwrite each other's records: the caller must order
+ * them, e.g. by issuing them on one stream. */
+#define DKS_STATIC_FIELD_MAX_NODES (1 << 18)
+int dks_field_at_particles_static(int nx, int ny, int nz, double hx, double hy, double hz, const double *phi_dev,
+                                  const double *x_dev, const double *y_dev, const double *z_dev, long long np, double ox, double oy,
+                                  double oz, double *epx_dev, double *epy_dev, double *epz_dev, void *stream);
+
 /* ---- One solve sharded over several GPUs (SURVEY.md sections 8(e), 8(f3)) ------------------------------------------------
  * The paper never splits a solve: several MPI ranks share ONE GPU through CUDA IPC.  This is the
  * contrasting B200 design: rank r of g (g a power of two <= 8; nx, ny, nz in [32, 256]) owns the y rows

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1108,6 +1109,86 @@ extern "C" int dks_poisson_solve_shard(dks_poisson_plan *p, int phase, const dou
     }
     default: return fail(DKS_ERR_INVALID_ARG, "phase must be 1, 2 or 3");
     }
+    DKS_CUDA(cudaGetLastError());
+    return DKS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// dks_field_at_particles_static: the field at the particles for callers that cannot allocate device memory
+// ------------------------------------------------------------------------------------------------
+// dks_field_at_particles keeps the node field (one 32-byte record per node) in the plan's buffer B, and a plan means
+// cudaMalloc: the twiddle tables on first use, and the workspace unless the caller brings one.  Some users of this
+// library cannot go there.  Examples: a tracking loop in which a cudaMalloc or cudaFree would stall every other stream
+// of the process (both synchronise the whole device); a host code whose own pool has already reserved all device
+// memory, so that a fresh cudaMalloc simply fails; a plug-in that is handed device pointers by its host and owns no
+// allocator.  For them the record array below lives in the library image itself.  Its price: every GPU on which this
+// library's module gets loaded holds these 8 MiB until the process exits, used or not, which is why the limit is modest.
+//
+// g_field_scratch is a __device__ symbol.  In host code its name is a host-side shadow, NOT a device address (a kernel
+// handed &g_field_scratch from the host would fault, or on systems where the GPU can reach host memory scribble over
+// host memory), so the host asks the runtime for the address, once per device and with that device current.
+static __device__ __align__(256) double g_field_scratch[4 * (size_t)DKS_STATIC_FIELD_MAX_NODES];
+
+static const int kStaticMaxDevices = 64;
+struct StaticScratchSlot { double4 *ptr = nullptr; int sm_count = 0; bool ready = false; };
+static StaticScratchSlot g_static_slot[kStaticMaxDevices];
+static std::mutex g_static_mutex;
+
+// Set-up of the current device, done by the first call on it: architecture check, SM count, device address of the array.
+// Neither call below allocates (the array came with the module).
+static int static_scratch_of_current_device(StaticScratchSlot *out)
+{
+    int dev = -1;
+    DKS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device ordinal %d is outside [0, %d)", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticScratchSlot &s = g_static_slot[dev];
+    if (!s.ready) {
+        int major = 0, sms = 0;
+        DKS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        DKS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (major != 10)
+            return fail(DKS_ERR_UNSUPPORTED_DEVICE, "device %d is compute capability %d.x; this library is built for sm_100a only", dev, major);
+        void *addr = nullptr;
+        DKS_CUDA(cudaGetSymbolAddress(&addr, g_field_scratch));
+        if (!addr || reinterpret_cast<uintptr_t>(addr) % 256) return fail(DKS_ERR_CUDA, "cudaGetSymbolAddress gave %p for the field scratch", addr);
+        s.ptr = static_cast<double4 *>(addr); s.sm_count = sms; s.ready = true;
+    }
+    *out = s;
+    return DKS_OK;
+}
+
+extern "C" int dks_field_at_particles_static(int nx, int ny, int nz, double hx, double hy, double hz, const double *phi,
+                                             const double *x, const double *y, const double *z, long long np, double ox, double oy,
+                                             double oz, double *epx, double *epy, double *epz, void *stream)
+{
+    if (!is_pow2_in_range(nx) || !is_pow2_in_range(ny) || !is_pow2_in_range(nz))
+        return fail(DKS_ERR_INVALID_ARG, "mesh %dx%dx%d: every extent must be a power of two in [8, 1024]", nx, ny, nz);
+    const long long nodes = (long long)nx * ny * nz;
+    if (nodes > (long long)DKS_STATIC_FIELD_MAX_NODES)
+        return fail(DKS_ERR_INVALID_ARG, "mesh %dx%dx%d has %lld nodes; dks_field_at_particles_static holds at most %lld "
+                    "(DKS_STATIC_FIELD_MAX_NODES, e.g. 64x64x64): use dks_field_at_particles with a plan for larger meshes",
+                    nx, ny, nz, nodes, (long long)DKS_STATIC_FIELD_MAX_NODES);
+    if (!(hx > 0) || !(hy > 0) || !(hz > 0) || !std::isfinite(hx) || !std::isfinite(hy) || !std::isfinite(hz))
+        return fail(DKS_ERR_INVALID_ARG, "spacings must be finite and > 0 (got %g, %g, %g)", hx, hy, hz);
+    if (!phi || np < 0 || (np > 0 && (!x || !y || !z || !epx || !epy || !epz)))
+        return fail(DKS_ERR_INVALID_ARG, "phi or a particle array is NULL, or np < 0");
+    if (!std::isfinite(ox) || !std::isfinite(oy) || !std::isfinite(oz)) return fail(DKS_ERR_INVALID_ARG, "origin must be finite");
+    StaticScratchSlot s;
+    int rc = static_scratch_of_current_device(&s);
+    if (rc) return rc;
+    if (np == 0) return DKS_OK;
+    MeshDims d = MeshDims();                                   // the two kernels read nx, ny, nz only
+    d.nx = nx; d.ny = ny; d.nz = nz;
+    ParticleFrame f;
+    f.ox = ox; f.oy = oy; f.oz = oz; f.hx = hx; f.hy = hy; f.hz = hz;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // Nothing in the array has to start at zero: the first kernel writes the record of every node of this mesh and the
+    // second reads only those, so whatever the previous call (of any mesh shape) left behind is never seen.
+    gradient_aos_kernel<<<dim3((nx + 127) / 128, ny, nz), 128, 0, st>>>(phi, s.ptr, d, 0.5 / hx, 0.5 / hy, 0.5 / hz);
+    const long long blocks = (np + 255) / 256;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(blocks, (long long)s.sm_count * 8 * 4));
+    gather_aos_kernel<<<grid, 256, 0, st>>>(s.ptr, x, y, z, np, f, d, epx, epy, epz);
     DKS_CUDA(cudaGetLastError());
     return DKS_OK;
 }

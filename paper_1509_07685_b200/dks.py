@@ -50,6 +50,7 @@ SYMBOLS = {
     "dks_gradient": (_i, [_vp, _vp, _vp, _vp, _vp, _vp]),
     "dks_gather_field": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "dks_field_at_particles": (_i, [_vp, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
+    "dks_field_at_particles_static": (_i, [_i, _i, _i, _d, _d, _d, _vp, _vp, _vp, _vp, C.c_longlong, _d, _d, _d, _vp, _vp, _vp, _vp]),
     "dks_poisson_set_shard": (_i, [_vp, _i, _i]),
     "dks_poisson_shard_buffers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
     "dks_poisson_set_peers": (_i, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
@@ -219,6 +220,20 @@ def dks_gather_field(plan, ex, ey, ez, x, y, z, np_, origin, epx, epy, epz, stre
 def dks_field_at_particles(plan, phi, x, y, z, np_, origin, epx, epy, epz, stream=None):
     return _check(lib.dks_field_at_particles(plan, _ptr(phi), _ptr(x), _ptr(y), _ptr(z), int(np_), *(float(v) for v in origin),
                                              _ptr(epx), _ptr(epy), _ptr(epz), stream), "dks_field_at_particles")
+
+
+DKS_STATIC_FIELD_MAX_NODES = 1 << 18
+
+
+def dks_field_at_particles_static(n, h, phi, x, y, z, np_, origin, epx, epy, epz, stream=None):
+    """dks_field_at_particles for callers that must not allocate device memory (a loop that a cudaMalloc would stall, a
+    host program whose pool owns the whole device, a component without an allocator): no plan; the node field goes through
+    an 8 MiB array inside the library, so nx * ny * nz <= DKS_STATIC_FIELD_MAX_NODES.  Calls on one device share that
+    array: do not let two of them overlap on the GPU.  n = (nx, ny, nz), h = (hx, hy, hz); everything else as in
+    dks_field_at_particles.  This wrapper only passes the pointers on; the outputs are the caller's."""
+    return _check(lib.dks_field_at_particles_static(*(int(v) for v in n), *(float(v) for v in h), _ptr(phi), _ptr(x), _ptr(y),
+                                                    _ptr(z), int(np_), *(float(v) for v in origin), _ptr(epx), _ptr(epy),
+                                                    _ptr(epz), stream), "dks_field_at_particles_static")
 
 
 def dks_poisson_set_shard(plan, rank, nranks):
