@@ -245,6 +245,56 @@ def test_p8_imag_zero_and_ghat_real_even(oracle, workloads):
     assert st["max_even_defect"] <= 1e-13 * st["max_abs"]
 
 
+# ----------------------------------------------------------------------------- P13: the Green's-octant accessor
+def mirrored_green_numpy(n, h, g0):
+    """Gt on the doubled grid, [2nz][2ny][2nx]: G at the mirrored index min(i, 2n - i), typed here in numpy."""
+    nx, ny, nz = n
+    ix = np.minimum(np.arange(2 * nx), 2 * nx - np.arange(2 * nx)) * h[0]
+    iy = np.minimum(np.arange(2 * ny), 2 * ny - np.arange(2 * ny)) * h[1]
+    iz = np.minimum(np.arange(2 * nz), 2 * nz - np.arange(2 * nz)) * h[2]
+    r = np.sqrt(iz[:, None, None] ** 2 + iy[None, :, None] ** 2 + ix[None, None, :] ** 2)
+    with np.errstate(divide="ignore"):
+        g = K_COULOMB / r
+    g[0, 0, 0] = g0
+    return g
+
+
+@pytest.mark.parametrize("n,h", [((4, 8, 2), (1e-3, 2e-3, 5e-4)), ((8, 2, 4), (3e-4, 1e-3, 2e-3)), ((2, 4, 16), (1e-3, 7e-4, 4e-4))])
+@pytest.mark.parametrize("precision", ["ld", "d"])
+def test_p13_ghat_octant_accessor(oracle, n, h, precision):
+    """Plan.ghat_octant() (oracle_*_plan_ghat_octant, the reference of the GPU test of step a0) is FT{Gt}[k, j, i] for k <= nz,
+    j <= ny, i <= nx, shape (nz+1, ny+1, nx+1).  Non-cubic, anisotropic
+    meshes: a swapped extent, stride or axis cannot cancel.  Two opinions: numpy.fft.fftn of Gt built in numpy, and the
+    oracle's O(L^2) definition dft1d applied axis by axis to the same Gt."""
+    nx, ny, nz = n
+    g0 = 0.37 * oracle.default_g0(h)                      # an override, so that the g0 argument is covered too
+    pl = oracle.Plan(n, h, g0=g0, precision=precision)
+    try:
+        oct_ = pl.ghat_octant()
+    finally:
+        pl.close()
+    assert oct_.shape == (nz + 1, ny + 1, nx + 1)
+    gt = mirrored_green_numpy(n, h, g0)
+    full = np.fft.fftn(gt)                                # (a) library transform, third opinion
+    scale = np.max(np.abs(full))
+    assert np.max(np.abs(full.imag)) <= 1e-13 * scale     # real and even: the octant carries everything
+    assert np.max(np.abs(oct_ - full.real[:nz + 1, :ny + 1, :nx + 1])) <= 1e-13 * scale
+    # (b) the definition, axis by axis (x, then y, then z), through the oracle's own O(L^2) dft1d
+    t = gt.astype(np.complex128)
+    for axis in (2, 1, 0):
+        t = np.apply_along_axis(lambda line: oracle.fft1d(line, sign=-1, precision=precision, definition=True), axis, t)
+    assert np.max(np.abs(t.imag)) <= 1e-13 * scale
+    assert np.max(np.abs(oct_ - t.real[:nz + 1, :ny + 1, :nx + 1])) <= 1e-13 * scale
+    # negative controls: the entries the accessor could pick by mistake are really different
+    for wrong in (full.real[1:nz + 2, :ny + 1, :nx + 1], full.real[:nz + 1, 1:ny + 2, :nx + 1], full.real[:nz + 1, :ny + 1, 1:nx + 2]):
+        assert np.max(np.abs(oct_ - wrong)) > 1e-3 * scale
+    wrong_pitch = full.real.ravel()[:oct_.size].reshape(oct_.shape)       # octant read with the doubled grid's own pitch
+    assert np.max(np.abs(oct_ - wrong_pitch)) > 1e-3 * scale
+    # and the even symmetry that lets the octant stand for the whole transform
+    k, j, i = nz // 2 or 1, ny // 2 or 1, nx // 2 or 1
+    assert abs(full.real[2 * nz - k, 2 * ny - j, 2 * nx - i] - oct_[k, j, i]) <= 1e-13 * scale
+
+
 # ----------------------------------------------------------------------------- P9: positivity
 def test_p9_positivity(oracle, workloads):
     n, h = (16, 16, 8), (1e-3, 1e-3, 1e-3)
