@@ -4,7 +4,9 @@
 
 produces oracle/liboracle_ld.so (REAL = long double: parity reference values) and
 oracle/liboracle_d.so (REAL = double: the timed CPU baseline) from oracle/poisson_oracle.c and oracle/field_ops_oracle.c.
-ORACLE_SANITIZE=1 adds -fsanitize=address,undefined (used by the sanitizer run recorded under profiles/).
+ORACLE_SANITIZE=1 adds -fsanitize=address,undefined (used by the sanitizer run recorded under profiles/) and writes to
+liboracle_ld_san.so / liboracle_d_san.so instead, so that an instrumented (several times slower) library can never be what a
+later run without the variable loads -- bench.py times the plain build as its CPU baseline.
 """
 from __future__ import annotations
 
@@ -14,7 +16,9 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRCS = [os.path.join(HERE, "poisson_oracle.c"), os.path.join(HERE, "field_ops_oracle.c")]
-LIBS = {"ld": os.path.join(HERE, "liboracle_ld.so"), "d": os.path.join(HERE, "liboracle_d.so")}
+SANITIZE = os.environ.get("ORACLE_SANITIZE") == "1"
+_SUFFIX = "_san" if SANITIZE else ""
+LIBS = {"ld": os.path.join(HERE, f"liboracle_ld{_SUFFIX}.so"), "d": os.path.join(HERE, f"liboracle_d{_SUFFIX}.so")}
 
 
 def _stale(lib: str) -> bool:
@@ -30,7 +34,7 @@ def build(force: bool = False) -> dict:
                "-Wall", "-Wextra"] + SRCS + ["-o", lib, "-lm"]
         if kind == "ld":
             cmd.insert(1, "-DORACLE_LD")
-        if os.environ.get("ORACLE_SANITIZE") == "1":
+        if SANITIZE:
             cmd[1:1] = ["-fsanitize=address,undefined", "-fno-omit-frame-pointer", "-g"]
         subprocess.run(cmd, check=True)
     return LIBS
