@@ -122,9 +122,16 @@ int dks_poisson_set_spacing(dks_poisson_plan *plan, double hx, double hy, double
 int dks_poisson_set_g0(dks_poisson_plan *plan, double g0_or_nan);
 
 /* Bytes of device workspace the plan needs (buffer A, the Green's octant, the three host-path staging
- * meshes, one slab of B).  "Memory management is left up to the user": the caller may allocate it
+ * meshes unless switched off, one slab of B).  "Memory management is left up to the user": the caller may allocate it
  * (Fig. 2's allocateMemory) and attach it with dks_poisson_set_workspace.  Host-only. */
 size_t dks_poisson_workspace_bytes(const dks_poisson_plan *plan);
+
+/* The host path (dks_poisson_solve_host*, dks_poisson_step_host_async) stages rho / phi in three mesh-sized buffers inside the
+ * workspace (3 x 8 nx ny nz bytes: 403 MB at 256^3).  A caller whose meshes stay on the device (PAPER.md:160 is the argument for
+ * that) can leave them out: enabled = 0 shrinks dks_poisson_workspace_bytes() accordingly and makes the host-path calls fail
+ * with DKS_ERR_NOT_SETUP.  Default: enabled.  Call it before the workspace is attached / before dks_greens_setup
+ * (DKS_ERR_INVALID_ARG afterwards).  Sharded plans never carry the staging buffers and refuse the host path.  Host-only. */
+int dks_poisson_set_host_staging(dks_poisson_plan *plan, int enabled);
 
 /* Attaches caller-owned device memory (e.g. a torch tensor) as the workspace (Fig. 2);
  * 256-byte aligned, at least dks_poisson_workspace_bytes() (else DKS_ERR_WORKSPACE_TOO_SMALL).  The caller keeps
@@ -229,7 +236,7 @@ int dks_field_at_particles_static(int nx, int ny, int nz, double hx, double hy, 
 
 /* ---- One solve sharded over several GPUs (SURVEY.md sections 8(e), 8(f3)) ------------------------------------------------
  * The paper never splits a solve: several MPI ranks share ONE GPU through CUDA IPC.  This is the
- * contrasting B200 design: rank r of g (g a power of two <= 8; nx, ny, nz in [32, 256]) owns the y rows
+ * contrasting B200 design: rank r of g (g a power of two <= 8; nx, ny, nz in [16, 256]) owns the y rows
  * [r ny/g, (r+1) ny/g) of rho and phi and the half-spectrum planes kz in [r nz/g, (r+1) nz/g) (the last rank also plane
  * nz).  P1 runs on the y slab and stores every output row directly into the receive buffer of the rank that owns its
  * plane; P2, P3, P4 run on the kz slab and P4 stores every row into the receive buffer of the rank that owns its y row;
@@ -238,10 +245,12 @@ int dks_field_at_particles_static(int nx, int ny, int nz, double hx, double hy, 
  * all-to-alls of buffer A, 2 x 269 MB at 256^3 -- are the epilogues of the producing kernels, not separate collectives.
  * Between the phases the caller runs its own inter-rank barrier (e.g. an NCCL barrier on the same stream).
  *
- *   dks_poisson_set_shard     before the workspace is attached; changes dks_poisson_workspace_bytes()
+ *   dks_poisson_set_shard     before the workspace is attached; changes dks_poisson_workspace_bytes(); afterwards
+ *                             dks_poisson_set_max_batch (> 1) and dks_poisson_set_slab_planes are refused
  *   dks_greens_setup          every rank builds the full Green's octant (it only reads its own planes)
  *   dks_poisson_shard_buffers this rank's two receive buffers (inside its workspace), to be published to the peers
- *   dks_poisson_set_peers     tables of all ranks' receive buffers as seen from this device (entry `rank` = its own)
+ *   dks_poisson_set_peers     tables of all ranks' receive buffers as seen from this device (entry `rank` = its own);
+ *                             each table must hold nranks entries (the library reads exactly that many)
  *   dks_poisson_solve_shard   phase 1 (P1), barrier, phase 2 (P2-P4), barrier, phase 3 (P5); rho_loc / phi_loc are this
  *                             rank's y slabs, [nz][ny/g][nx] contiguous fp64 (rho_loc for phase 1, phi_loc for phase 3)
  * A sharded plan refuses dks_poisson_solve. */

@@ -89,6 +89,7 @@ struct dks_poisson_plan {
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_in[kHostSlots] = {}, ev_solve[kHostSlots] = {}, ev_out[kHostSlots] = {};
     unsigned long long host_calls = 0;
+    bool host_staging = true;           // the workspace carries the kHostSlots staging meshes (dks_poisson_set_host_staging; never on sharded plans)
     size_t offA, offB, offG, offS, need_bytes;
     // P2..P4 run slab by slab (slab = `slab` consecutive kz planes) so that B, the largest intermediate,
     // is a slab-sized scratch that stays resident in L2 between the three passes
@@ -114,6 +115,8 @@ struct dks_poisson_plan {
     cudaEvent_t setup_done = nullptr;
     cudaEvent_t ghat_free = nullptr;    // recorded after the last P3 of a solve that runs on another stream than the setup:
     bool ghat_free_recorded = false;    // the next rebuild of Ghat waits for it
+    bool ghat_read_on_setup_stream = false;   // a solve ran on setup_used since the last rebuild: no event was recorded for it (stream
+                                              // order covers a rebuild on that stream); a rebuild that moves to another stream records one then
     // profiling
     int prof_slots = 0;                 // 0 = off; else per-pass events of the last prof_slots solves are kept
     long long prof_count = 0;           // profiled solves issued since profiling was switched on
@@ -164,7 +167,8 @@ static void compute_layout(dks_poisson_plan *p)
         p->offA = off; off = align_up(off + 16 * nx * ny * (nz + 1) * nbm, 256);
     }
     p->offG = off; off = align_up(off + 8 * (size_t)p->d.gpitch * (ny + 1) * (nz + 1), 256);
-    p->offS = off; off = align_up(off + kHostSlots * align_up(8 * nx * ny * nz, 256), 256);
+    p->offS = off;
+    if (p->host_staging && p->nranks == 1) off = align_up(off + kHostSlots * align_up(8 * nx * ny * nz, 256), 256);
     p->offB = off; off = align_up(off + 16 * nx * 2 * ny * (size_t)(p->nranks > 1 ? p->planes_loc : p->slab) * nbm, 256);
     p->need_bytes = off;
     p->steps.clear();
@@ -524,6 +528,7 @@ extern "C" int dks_poisson_set_slab_planes(dks_poisson_plan *p, int planes)
 {
     if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
     if (planes < 0 || planes > p->d.nz + 1) return fail(DKS_ERR_INVALID_ARG, "planes must be in [0, nz+1] (0 = automatic)");
+    if (p->nranks > 1) return fail(DKS_ERR_INVALID_ARG, "sharding excludes slabs (this plan is rank %d of %d)", p->rank, p->nranks);
     const int old = p->slab;
     p->slab = planes ? planes : auto_slab(p);
     compute_layout(p);
@@ -585,8 +590,20 @@ static int greens_setup_on(dks_poisson_plan *p, cudaStream_t st)
         bind_workspace(p);
     }
     const MeshDims d = p->d;
-    // the rebuild overwrites Ghat: order it after the last P3 issued on another stream (P3 is the only reader of Ghat)
+    // The rebuild overwrites Ghat in place, in three passes.  Order it after (1) the last P3 issued on another stream (P3 is the
+    // only reader of Ghat), (2) a previous build still running on another stream, (3) solves that ran on the previous build's own
+    // stream: those record no event per solve (it would sit between P3 and P4 of every solve), so one is recorded now, at the
+    // current tail of that stream -- behind the whole solve, which is more than needed but happens once per change of stream.
     if (p->ghat_free_recorded) DKS_CUDA(cudaStreamWaitEvent(st, p->ghat_free, 0));
+    if (st != p->setup_used) {
+        if (p->setup_pending) DKS_CUDA(cudaStreamWaitEvent(st, p->setup_done, 0));
+        if (p->ghat_read_on_setup_stream) {
+            DKS_CUDA(cudaEventRecord(p->ghat_free, p->setup_used));
+            DKS_CUDA(cudaStreamWaitEvent(st, p->ghat_free, 0));
+            p->ghat_free_recorded = true;
+        }
+    }
+    p->ghat_read_on_setup_stream = false;
     // 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), evaluated in long double.
     const long double pi_l = 3.141592653589793238462643383279502884L;
     const double coef = (double)(1.0L / (4.0L * pi_l * 8.8541878128e-12L));
@@ -760,6 +777,18 @@ static bool last_p3(const dks_poisson_plan *p, size_t i)
     return true;
 }
 
+// Called right after the last P3 of a solve on `st`: a later rebuild of Ghat must not overtake it.
+static int note_ghat_read(dks_poisson_plan *p, cudaStream_t st)
+{
+    if (st != p->setup_used) {
+        DKS_CUDA(cudaEventRecord(p->ghat_free, st));
+        p->ghat_free_recorded = true;
+    } else {
+        p->ghat_read_on_setup_stream = true;     // greens_setup_on records the event if the rebuild ever moves to another stream
+    }
+    return DKS_OK;
+}
+
 static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int nb, void *stream)
 {
     if (!p || !rho || !phi) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
@@ -801,9 +830,9 @@ static int solve_impl(dks_poisson_plan *p, const double *rho, double *phi, int n
         else if (p->big[s.pass - 1] == 2048) launch_big<2048>(s, p, rho, phi, nb, st);
         else launch_generic(s, p, rho, phi, nb, st);
         // a later rebuild of Ghat on the setup stream must not overtake this solve's last P3
-        if (s.pass == 3 && last_p3(p, i) && st != p->setup_used && !capturing) {
-            DKS_CUDA(cudaEventRecord(p->ghat_free, st));
-            p->ghat_free_recorded = true;
+        if (s.pass == 3 && last_p3(p, i) && !capturing) {
+            int rc = note_ghat_read(p, st);
+            if (rc) return rc;
         }
     }
     if (prof) { DKS_CUDA(cudaEventRecord(ev[p->steps.size()], st)); ++p->prof_count; }
@@ -825,6 +854,7 @@ extern "C" int dks_poisson_set_max_batch(dks_poisson_plan *p, int nbatch)
 {
     if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
     if (nbatch < 1 || nbatch > 64) return fail(DKS_ERR_INVALID_ARG, "nbatch must be in [1, 64]");
+    if (p->nranks > 1 && nbatch != 1) return fail(DKS_ERR_INVALID_ARG, "sharding excludes batches (this plan is rank %d of %d)", p->rank, p->nranks);
     if ((long long)(p->d.nz + 1) * nbatch > 65535)      // P2 / P4 put (plane, mesh) on gridDim.y
         return fail(DKS_ERR_INVALID_ARG, "(nz + 1) * nbatch = %lld exceeds 65535 (grid limit of the y passes)", (long long)(p->d.nz + 1) * nbatch);
     const int old = p->max_batch;
@@ -842,12 +872,23 @@ extern "C" int dks_poisson_set_max_batch(dks_poisson_plan *p, int nbatch)
     return DKS_OK;
 }
 
+extern "C" int dks_poisson_set_host_staging(dks_poisson_plan *p, int enabled)
+{
+    if (!p) return fail(DKS_ERR_INVALID_ARG, "plan is NULL");
+    if (p->ws) return fail(DKS_ERR_INVALID_ARG, "dks_poisson_set_host_staging must be called before the workspace is attached / before dks_greens_setup");
+    p->host_staging = enabled != 0;
+    compute_layout(p);
+    return DKS_OK;
+}
+
 // Host path.  Every call copies its rho to the device, solves and copies phi back, but consecutive calls
 // overlap: the copy-in of call i+1 and the copy-out of call i-1 run on their own streams beside the solve
 // of call i (PCIe is full duplex), as PAPER.md:132 does for the rho transfer.  kHostSlots staging meshes take turns.
 extern "C" int dks_poisson_solve_host_async(dks_poisson_plan *p, const double *rho_host, double *phi_host, void *stream)
 {
     if (!p || !rho_host || !phi_host) return fail(DKS_ERR_INVALID_ARG, "plan, rho or phi is NULL");
+    if (p->nranks > 1) return fail(DKS_ERR_INVALID_ARG, "this plan is one rank of a sharded solve: it has no host path");
+    if (!p->host_staging) return fail(DKS_ERR_NOT_SETUP, "the host path was switched off for this plan (dks_poisson_set_host_staging)");
     if (!p->greens_ready) return fail(DKS_ERR_NOT_SETUP, "call dks_greens_setup before dks_poisson_solve_host");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (!p->s_in) {
@@ -1004,7 +1045,7 @@ extern "C" int dks_poisson_set_shard(dks_poisson_plan *p, int rank, int nranks)
     if (p->ws) return fail(DKS_ERR_INVALID_ARG, "dks_poisson_set_shard must be called before the workspace is attached / before dks_greens_setup");
     if (nranks > 1) {
         if (!(p->fast[0] && p->fast[1] && p->fast[2]))
-            return fail(DKS_ERR_INVALID_ARG, "a sharded solve needs nx, ny, nz in [32, 256] (register-resident passes on every axis)");
+            return fail(DKS_ERR_INVALID_ARG, "a sharded solve needs nx, ny, nz in [16, 256] (register-resident passes on every axis)");
         if (p->d.ny / nranks < 1 || p->d.nz / nranks < 1) return fail(DKS_ERR_INVALID_ARG, "more ranks than rows");
         if (p->max_batch != 1 || p->slab != p->d.nz + 1) return fail(DKS_ERR_INVALID_ARG, "sharding excludes batches and slabs");
     }
@@ -1089,6 +1130,7 @@ extern "C" int dks_poisson_solve_shard(dks_poisson_plan *p, int phase, const dou
         dks_poisson_plan::Step s2 = { 2, 0, p->planes_loc }, s3 = { 3, p->kz0, p->planes_loc };
         launch_r16(s2, p, nullptr, nullptr, 1, st);            // reads A1 (= p->A, local planes), writes B
         launch_r16(s3, p, nullptr, nullptr, 1, st);            // Ghat planes kz0 ..
+        { int rc = note_ghat_read(p, st); if (rc) return rc; }
         switch (p->r16A[1]) {
 #define X(A_) case A_: shard_launch_p4<A_>(p, st); break;
             DKS_FOR_EACH_A(X)

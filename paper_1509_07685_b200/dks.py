@@ -37,6 +37,7 @@ SYMBOLS = {
     "dks_poisson_set_g0": (_i, [_vp, _d]),
     "dks_poisson_workspace_bytes": (_sz, [_vp]),
     "dks_poisson_set_workspace": (_i, [_vp, _vp, _sz]),
+    "dks_poisson_set_host_staging": (_i, [_vp, _i]),
     "dks_poisson_set_stream": (_i, [_vp, _vp]),
     "dks_poisson_set_slab_planes": (_i, [_vp, _i]),
     "dks_poisson_slab_planes": (_i, [_vp]),
@@ -165,6 +166,10 @@ def dks_poisson_set_workspace(plan, dev, nbytes=None):
     return _check(lib.dks_poisson_set_workspace(plan, _ptr(dev), int(nbytes)), "dks_poisson_set_workspace")
 
 
+def dks_poisson_set_host_staging(plan, enabled):
+    return _check(lib.dks_poisson_set_host_staging(plan, int(bool(enabled))), "dks_poisson_set_host_staging")
+
+
 def dks_poisson_set_stream(plan, stream):
     return _check(lib.dks_poisson_set_stream(plan, stream), "dks_poisson_set_stream")
 
@@ -223,6 +228,7 @@ def dks_field_at_particles(plan, phi, x, y, z, np_, origin, epx, epy, epz, strea
 
 
 DKS_STATIC_FIELD_MAX_NODES = 1 << 18
+MAX_RANKS = 8                          # kMaxRanks in csrc/dks_passes_r16.cuh
 
 
 def dks_field_at_particles_static(n, h, phi, x, y, z, np_, origin, epx, epy, epz, stream=None):
@@ -247,8 +253,13 @@ def dks_poisson_shard_buffers(plan):
 
 
 def dks_poisson_set_peers(plan, recv_p1_of_rank, recv_p4_of_rank):
-    n = len(recv_p1_of_rank)
-    t1, t2 = (_vp * n)(*recv_p1_of_rank), (_vp * n)(*recv_p4_of_rank)
+    # The C side reads one entry per rank and does not know the tables' lengths: pad both to the largest rank count the library
+    # supports (8) with NULL, which it rejects by rank number, so a table that is too short is an error instead of a wild read.
+    n1, n2 = len(recv_p1_of_rank), len(recv_p4_of_rank)
+    if n1 != n2 or not 2 <= n1 <= MAX_RANKS:
+        raise ValueError(f"peer tables must have the same length in [2, {MAX_RANKS}] (got {n1} and {n2})")
+    t1 = (_vp * MAX_RANKS)(*recv_p1_of_rank, *([None] * (MAX_RANKS - n1)))
+    t2 = (_vp * MAX_RANKS)(*recv_p4_of_rank, *([None] * (MAX_RANKS - n2)))
     return _check(lib.dks_poisson_set_peers(plan, t1, t2), "dks_poisson_set_peers")
 
 
@@ -260,7 +271,7 @@ def dks_poisson_solve_shard(plan, phase, rho_loc, phi_loc, stream=None):
 class PoissonPlan:
     """Owns a dks_poisson_plan and a torch-allocated workspace on the current CUDA device."""
 
-    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, max_batch=None):
+    def __init__(self, n, h, g0=None, own_workspace=True, slab_planes=None, max_batch=None, host_staging=True):
         import torch
 
         self.n, self.h = tuple(int(v) for v in n), tuple(float(v) for v in h)
@@ -272,6 +283,8 @@ class PoissonPlan:
             dks_poisson_set_slab_planes(self._plan, slab_planes)
         if max_batch is not None:
             dks_poisson_set_max_batch(self._plan, max_batch)
+        if not host_staging:
+            dks_poisson_set_host_staging(self._plan, False)
         if own_workspace:
             nbytes = dks_poisson_workspace_bytes(self._plan)
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")

@@ -126,3 +126,41 @@ def test_host_only_plan_options(dks):
             "p1_z_r2c_r16p", "p2_y_fwd_r16p", "p3_x_conv_r16", "p4_y_inv_r16", "p5_z_c2r_r16"]   # n = 128: one CTA per parity
     finally:
         dks.dks_poisson_plan_destroy(q)
+
+
+def test_host_staging_and_shard_options(dks):
+    """The host-path staging meshes are optional; sharded plans carry none and refuse batches and slabs."""
+    nx, ny, nz = 64, 64, 32
+    mesh = 8 * nx * ny * nz
+    p = dks.dks_poisson_plan_create(nx, ny, nz, 1e-4, 1e-4, 1e-4)
+    try:
+        ws = dks.dks_poisson_workspace_bytes(p)
+        dks.dks_poisson_set_host_staging(p, False)
+        assert ws - dks.dks_poisson_workspace_bytes(p) == 3 * mesh              # three staging meshes (already 256-byte multiples)
+        dks.dks_poisson_set_host_staging(p, True)
+        assert dks.dks_poisson_workspace_bytes(p) == ws
+        dks.dks_poisson_set_host_staging(p, False)
+        dks.dks_poisson_set_shard(p, 1, 2)                                      # rank 1 of 2: A1 + A2 + Ghat + B(local planes)
+        a1, a2 = 16 * nx * ny * (nz // 2 + 1), 16 * nx * (ny // 2) * (nz + 1)
+        ghat = 8 * ((nx + 1 + 7) // 8 * 8) * (ny + 1) * (nz + 1)
+        expect = a1 + a2 + ghat + 2 * a1
+        assert 0 <= dks.dks_poisson_workspace_bytes(p) - expect <= 4 * 256
+        dks.dks_poisson_set_host_staging(p, True)                               # no staging on a sharded plan either way
+        assert 0 <= dks.dks_poisson_workspace_bytes(p) - expect <= 4 * 256
+        before = dks.dks_poisson_workspace_bytes(p)
+        for call in (lambda: dks.dks_poisson_set_max_batch(p, 2), lambda: dks.dks_poisson_set_slab_planes(p, 4)):
+            with pytest.raises(dks.DksError) as e:
+                call()
+            assert e.value.status == dks.DKS_ERR_INVALID_ARG and "sharding excludes" in str(e.value)
+        assert dks.dks_poisson_workspace_bytes(p) == before
+        dks.dks_poisson_set_max_batch(p, 1)                                     # the default stays acceptable
+        for t1, t2 in [([1, 2], [1]), ([1], [1]), ([1] * 9, [1] * 9)]:          # table lengths are checked before the C call
+            with pytest.raises(ValueError):
+                dks.dks_poisson_set_peers(p, t1, t2)
+    finally:
+        dks.dks_poisson_plan_destroy(p)
+    q = dks.dks_poisson_plan_create(16, 16, 16, 1e-3, 1e-3, 1e-3)               # the smallest extent a sharded solve takes
+    try:
+        dks.dks_poisson_set_shard(q, 0, 2)
+    finally:
+        dks.dks_poisson_plan_destroy(q)

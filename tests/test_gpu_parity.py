@@ -395,6 +395,35 @@ def test_rebuild_on_side_stream_between_pipelined_solves(torch_cuda, dks, oracle
         plan.close()
 
 
+def test_rebuild_moves_to_another_stream_behind_queued_solves(torch_cuda, dks, oracle, workloads):
+    # PoissonPlan(h0) builds Ghat on torch's current stream and the solves below run there too, so no solve records an event.
+    # step_host_async(h1) then moves the rebuild to the plan's own stream while those solves are still queued: it must wait
+    # for the first build and for the last queued P3 (it overwrites Ghat in place), with no host synchronisation in between.
+    torch = torch_cuda
+    n = (128, 128, 128)
+    h0, h1 = (1e-4, 2e-4, 3e-4), (2.5e-4, 1.5e-4, 0.7e-4)
+    rho0, rho1 = workloads.random_rho(n, seed=71), workloads.random_rho(n, seed=72)
+    ref0 = oracle.solve(rho0, n, h0, precision="d")
+    ref1 = oracle.solve(rho1, n, h1, precision="d")
+    d_rho0 = torch.from_numpy(rho0).cuda()
+    phis = [torch.empty_like(d_rho0) for _ in range(24)]
+    h_in, h_out = torch.from_numpy(rho1).pin_memory(), torch.empty(rho1.shape, dtype=torch.float64).pin_memory()
+    torch.cuda.synchronize()
+    plan = dks.PoissonPlan(n, h0)
+    try:
+        for phi in phis:                       # about 2.5 ms of queued work, all of it reading the h0 transform
+            plan.solve(d_rho0, phi)
+        plan.step_host_async(h1, h_in, h_out)
+        plan.host_sync()
+        torch.cuda.synchronize()
+        check(phis[-1].cpu().numpy(), ref0)
+        check(phis[0].cpu().numpy(), ref0)
+        assert all(torch.equal(phis[0], phi) for phi in phis[1:])
+        check(h_out.numpy(), ref1)
+    finally:
+        plan.close()
+
+
 def test_two_live_plans_of_different_shapes(torch_cuda, dks, oracle, workloads):
     # the kernels' shared-memory attributes are process-wide: a small plan must not lower what a large one needs
     torch = torch_cuda
@@ -530,6 +559,34 @@ def test_caller_owned_and_plan_owned_workspace(torch_cuda, dks, oracle, workload
         assert e.value.status == dks.DKS_ERR_NOT_SETUP
     finally:
         dks.dks_poisson_plan_destroy(h_)
+
+
+def test_plan_without_host_staging(torch_cuda, dks, oracle, workloads):
+    # device-resident callers can leave the three staging meshes out of the workspace; the host path is then refused
+    torch = torch_cuda
+    n, h = (32, 16, 64), (2e-4, 3e-4, 1e-4)
+    rho = workloads.random_rho(n, seed=5)
+    full = dks.PoissonPlan(n, h)
+    plan = dks.PoissonPlan(n, h, host_staging=False)
+    try:
+        assert dks.dks_poisson_workspace_bytes(full.handle) - dks.dks_poisson_workspace_bytes(plan.handle) == 3 * rho.nbytes
+        with pytest.raises(dks.DksError):                      # the workspace is attached: too late to change its layout
+            dks.dks_poisson_set_host_staging(plan.handle, True)
+        d_rho = torch.from_numpy(rho).cuda()
+        phi = plan.solve(d_rho)
+        e = plan.field_at_particles(phi, d_rho.flatten()[:100].contiguous(), d_rho.flatten()[:100].contiguous(),
+                                    d_rho.flatten()[:100].contiguous(), (0.0, 0.0, 0.0))      # buffer B is still there
+        torch.cuda.synchronize()
+        assert torch.equal(phi, full.solve(d_rho))
+        check(phi.cpu().numpy(), oracle.solve(rho, n, h, precision="ld"))
+        out = np.empty_like(rho)
+        with pytest.raises(dks.DksError) as err:
+            plan.solve_host(rho, out)
+        assert err.value.status == dks.DKS_ERR_NOT_SETUP
+    finally:
+        torch.cuda.synchronize()
+        full.close()
+        plan.close()
 
 
 def test_long_line_passes_are_selected(dks):

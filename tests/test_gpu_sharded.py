@@ -10,7 +10,7 @@ pytestmark = pytest.mark.gpu
 REL_L2_TOL, MAX_ABS_TOL = 1e-12, 1e-11
 
 
-@pytest.mark.parametrize("n,g", [((32, 32, 32), 2), ((64, 64, 64), 4), ((32, 64, 128), 8), ((256, 32, 64), 2),
+@pytest.mark.parametrize("n,g", [((16, 16, 16), 2), ((16, 32, 64), 4), ((64, 16, 16), 8), ((32, 32, 32), 2), ((64, 64, 64), 4), ((32, 64, 128), 8), ((256, 32, 64), 2),
                                  ((128, 256, 32), 8), ((64, 32, 256), 4)])
 def test_emulated_sharded_solve(oracle, workloads, n, g):
     import torch
@@ -58,6 +58,9 @@ def test_shard_refusals():
             dks.dks_poisson_solve(h_, d, d, None)
         with pytest.raises(dks.DksError):                       # peers not set
             dks.dks_poisson_solve_shard(h_, 1, d, d, None)
+        with pytest.raises(dks.DksError) as e:                  # the host path does not exist on a sharded plan
+            dks.dks_poisson_solve_host(h_, d.cpu().numpy(), d.cpu().numpy(), None)
+        assert "no host path" in str(e.value)
     finally:
         torch.cuda.synchronize()
         dks.dks_poisson_plan_destroy(h_)
