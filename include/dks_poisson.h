@@ -41,6 +41,9 @@ typedef enum dks_status {
     DKS_ERR_INVALID_ARG = -1,        /* NULL pointer, n not a power of two in [8,1024], h <= 0 or not finite */
     DKS_ERR_UNSUPPORTED_DEVICE = -2, /* current device is not compute capability 10.x                      */
     DKS_ERR_WORKSPACE_TOO_SMALL = -4,/* dks_poisson_set_workspace: bytes < dks_poisson_workspace_bytes     */
+    /* -3 is not used: SURVEY.md section 8(b) lists a NO_WORKSPACE status; a plan without a workspace allocates its own in
+     * dks_greens_setup, so the only way to meet that state is to call an entry point before the set-up, and that is
+     * reported as DKS_ERR_NOT_SETUP (dks_field_at_particles, dks_poisson_shard_buffers, dks_poisson_set_peers). */
     DKS_ERR_NOT_SETUP = -5,          /* dks_poisson_solve before dks_greens_setup (or after a spacing change) */
     DKS_ERR_CUDA = -6                /* a CUDA runtime call failed; see dks_last_error()                   */
 } dks_status;
