@@ -36,6 +36,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index 1..5 (default 4 = 256^3)")
+    ap.add_argument("--mesh", type=int, nargs=3, metavar=("NX", "NY", "NZ"), default=None,
+                    help="context workload instead of a BASELINE config (never the headline): e.g. 512 512 256, the largest mesh of "
+                         "the paper's Table 1 (PAPER.md:157-158); uniform random rho, no CPU / cuFFT / particle legs")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=60, help="host-path steps per e2e loop (pipeline fill and drain are inside the timed region)")
     ap.add_argument("--slab", type=int, default=None, help="planes per P2-P4 slab (default: the plan's automatic choice)")
@@ -44,6 +47,7 @@ def parse():
     ap.add_argument("--no-cufft", action="store_true", help="skip the torch.fft (cuFFT) side reference")
     ap.add_argument("--ref-sample", action="store_true",
                     help="--impl reference: time the central half-extent sub-mesh instead of the full mesh (reported unscaled, under its own workload name)")
+    ap.add_argument("--field-reps", type=int, default=10, help="timed repetitions of each particle-kernel measurement (1 for ncu captures)")
     ap.add_argument("--repeats", type=int, default=5, help="timed windows of --steps solves each; the median is reported")
     ap.add_argument("--sustained-s", type=float, default=2.0, help="length of the additional back-to-back run (0 = skip)")
     return ap.parse_args()
@@ -276,10 +280,18 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = W.config(args.config)
-    # replicas only: every rank gets the same bunch shape from its own seed offset is not needed --
-    # run time is data independent; all ranks use the config's rho.
-    rho = W.make_rho(w)
+    if args.mesh:
+        nx_, ny_, nz_ = args.mesh
+        w = W.Workload(f"mesh_{nx_}x{ny_}x{nz_}", (nx_, ny_, nz_), (1e-4, 1e-4, 2e-4), 0, 7,
+                       "context workload (--mesh): uniform random rho, seed 7; run time is data independent")
+        rho = W.random_rho(w.n, seed=w.seed, signed=False)
+        args.no_cpu_baseline = args.no_cufft = True
+        args.e2e_steps = min(args.e2e_steps, 6)
+    else:
+        w = W.config(args.config)
+        # replicas only: every rank gets the same bunch shape from its own seed offset is not needed --
+        # run time is data independent; all ranks use the config's rho.
+        rho = W.make_rho(w)
     nbytes = rho.nbytes
     d_rho = torch.from_numpy(rho).cuda()
     d_phi = torch.empty_like(d_rho)
@@ -424,7 +436,7 @@ def run_ours(args):
     # ---- f4: the whole space-charge step with the particles resident on the device (deposit -> solve -> E -> gather):
     # nothing but a scalar crosses the host link (PAPER.md:160 names that link as the limiter)
     field_ops = None
-    if world == 1:
+    if world == 1 and not args.mesh:
         px, py, pz, pq, origin = W.particles(w)
         dpx, dpy, dpz, dpq = (torch.from_numpy(a).cuda() for a in (px, py, pz, pq))
         n_p = dpx.numel()
@@ -435,7 +447,7 @@ def run_ours(args):
             plan.solve(f_rho, d_phi)
             return plan.field_at_particles(d_phi, dpx, dpy, dpz, origin)
 
-        def timed(fn, reps=10):
+        def timed(fn, reps=args.field_reps):
             for _ in range(2):
                 fn()
             e0.record(stream)
@@ -457,6 +469,39 @@ def run_ours(args):
         field_ops["device_resident_step"] = {"ms_per_step": step_ms, "value": 1e3 / step_ms, "unit": "steps/s",
                                              "api": "dks_deposit_cic + dks_poisson_solve + dks_field_at_particles (= gradient + gather), "
                                                     "particles and meshes resident on the device; no host traffic"}
+        # the step as the paper runs it: the mesh follows the bunch, so the spacings change and the Green's
+        # transform is rebuilt every step (dks_poisson_set_spacing + dks_greens_setup on the same stream, inside the timed region)
+        calls = [0]
+
+        def space_charge_step_with_rebuild():
+            calls[0] += 1
+            plan.set_spacing(tuple(v * (1.0 + 1e-3 * (calls[0] % 7)) for v in w.h))
+            return space_charge_step()
+
+        step2_ms = timed(space_charge_step_with_rebuild)
+        plan.set_spacing(w.h)
+        field_ops["device_resident_step_with_greens_rebuild"] = {
+            "ms_per_step": step2_ms, "value": 1e3 / step2_ms, "unit": "steps/s",
+            "api": "dks_poisson_set_spacing + dks_greens_setup + dks_deposit_cic + dks_poisson_solve + dks_field_at_particles"}
+        # algorithmic bytes of the f4 kernels against the measured copy bandwidth; the particle kernels
+        # touch the mesh at random in generator order, so their floors assume every node is moved once
+        nodes = w.n[0] * w.n[1] * w.n[2]
+        peak_gbs = measured_peaks()[0]
+
+        def roof(ms, nbytes_alg):
+            gbs = nbytes_alg / (ms * 1e-3) / 1e9
+            return {"bound": "hbm", "ms": ms, "algorithmic_bytes": nbytes_alg, "achieved": gbs, "peak": peak_gbs, "unit": "GB/s",
+                    "frac": gbs / peak_gbs}
+
+        field_ops["roofline"] = {
+            "cic_deposit_kernel (+ memset of rho)": roof(field_ops["deposit_ms"], 32.0 * n_p + 16.0 * nodes),
+            "gradient_kernel": roof(field_ops["gradient_ms"], 32.0 * nodes),
+            "gather_field_kernel": roof(field_ops["gather_ms"], 48.0 * n_p + 24.0 * nodes),
+            "gradient_aos_kernel + gather_aos_kernel": roof(field_ops["field_at_particles_ms"], 48.0 * n_p + 72.0 * nodes),
+            "bytes": "deposit: 32 B/particle (x, y, z, q) + 8 B/node memset + 8 B/node of sums; gradient: 8 B/node read + 24 written; "
+                     "gather: 24 B/particle read + 24 written + 24 B/node; fused: 48 B/particle + 8 B/node phi + 32 B/node record "
+                     "written + 32 read",
+        }
         del dpx, dpy, dpz, dpq, f_rho, ex, ey, ez
 
     if rank != 0:
@@ -499,6 +544,12 @@ def run_ours(args):
                         "sustained_frac": m3 / (sustained["ms_per_step"] * 1e-3) / 1e9 / peak if sustained else None,
                         "sustained_frac_of_8TBs": m3 / (sustained["ms_per_step"] * 1e-3) / 8e12 if sustained else None},
     }
+    # a0 (dks_greens_setup: three kernels): the octant is written once by the x kernel and transformed in place along y and z
+    g_bytes = 8.0 * (w.n[0] + 1) * (w.n[1] + 1) * (w.n[2] + 1)
+    roofline["greens_setup"] = {"bound": "hbm", "ms": greens_ms, "algorithmic_bytes": 5 * g_bytes,
+                                "achieved": 5 * g_bytes / (greens_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                                "frac": 5 * g_bytes / (greens_ms * 1e-3) / 1e9 / peak,
+                                "bytes": "octant written once (x kernel, G evaluated on the fly) + read and written by the y and the z kernel"}
     plan.close()
 
     # ---- side reference (north_star: "cuFFT may be timed as a side reference"): the paper-style pipeline

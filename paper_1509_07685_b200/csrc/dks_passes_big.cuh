@@ -145,19 +145,33 @@ p5_z_c2r_big(const cplx *__restrict__ A, double *__restrict__ phi, MeshDims d, c
 // ---- P3: forward x, multiply by the Green's transform, inverse x, crop; in place; W consecutive lines per CTA -----------
 // The forward's stage 3, the multiplication and the inverse's stage 3 work on the same 16 registers.  The W Green's rows
 // are staged in shared memory behind the tile (coalesced row reads instead of scattered 8-byte gathers from L2).
+// Staged Green's rows: a warp reads them with lanes = (4 or 8 sets u) x (W lines w), and the frequencies of neighbouring sets
+// differ by multiples of 64 (L = 1024) or 32 (L = 2048) -- with plain rows of L/2 + 8 doubles all 32 lanes met in two banks
+// (ncu, 512 x 512 x 256: 1.2e8 conflicts per launch).  Entry k of a row therefore sits at k + (k >> SH) (injective up to
+// the Nyquist entry k = L/2, which lands at L/2 + 8 or + 32), and the row stride is 4 (W = 8) or 8 (W = 4) doubles past a
+// multiple of 16, which spreads (u, w) over all sixteen 8-byte banks.
+// W lines per CTA and one CTA per SM, as in the strided passes (tried in round 3: W = 4 with two CTAs per SM needs an unpadded
+// tile to keep the quarter-warp stage accesses conflict free and was slower, 3.83 against 3.56 ms at 512 x 512 x 256).
 template <int L>
 struct P3BigGeom {
-    static constexpr int GROW = L / 2 + 8;                    // doubles per staged Green's row
-    static constexpr int SMEM = BigGeom<L>::SMEMX + BigGeom<L>::W * GROW * (int)sizeof(double);
+    static constexpr int W = BigGeom<L>::W, WP = BigGeom<L>::WPX;
+    static constexpr int THREADS = BigGeom<L>::THREADS, MINB = 1;
+    static constexpr int SH = L == 1024 ? 6 : 5;
+    static constexpr int GROW = L == 1024 ? 532 : 1064;       // doubles per staged Green's row (> gpos(L/2))
+    static constexpr int SMEM = L * WP * (int)sizeof(cplx) + W * GROW * (int)sizeof(double);
+    static __device__ __forceinline__ int gpos(int k) { return k + (k >> SH); }
+    static_assert(GROW > L / 2 + ((L / 2) >> SH) && GROW % 16 == 32 / W, "Green's row stride");
+    static_assert(MINB * (SMEM + 1024) <= 227 * 1024, "shared memory per SM");
+    static_assert((L / 2) % THREADS == 0 && (L / 2 * W) % THREADS == 0 && W <= THREADS, "fill loops");
 };
 
 template <int L, bool PDL = false>
-__global__ void __launch_bounds__(BigGeom<L>::THREADS, 1)
+__global__ void __launch_bounds__(P3BigGeom<L>::THREADS, P3BigGeom<L>::MINB)
 p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d, int kz0, const cplx *__restrict__ tw)
 {
     extern __shared__ cplx s[];
     typedef BigGeom<L> G;
-    constexpr int W = G::W, WP = G::WPX, NT = G::THREADS, N = L / 2, GROW = P3BigGeom<L>::GROW;
+    constexpr int W = P3BigGeom<L>::W, WP = P3BigGeom<L>::WP, NT = P3BigGeom<L>::THREADS, N = L / 2, GROW = P3BigGeom<L>::GROW;
     typedef BigStage<L, WP> St;
     double *gs = reinterpret_cast<double *>(s + L * WP);
     const int ny = d.ny, tid = threadIdx.x, w = tid % W, u = tid / W;
@@ -165,14 +179,38 @@ p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
     const int kz = (kz0 + line0 / (2 * ny)) % (d.nz + 1), ky0 = line0 % (2 * ny);    // a batch repeats kz
     cplx *base = B + (size_t)line0 * N;
     if (PDL) pdl_wait();
-#pragma unroll 4
-    for (int idx = tid; idx < N * W; idx += NT) {
-        const int ww = idx / N, pp = idx % N;
-        s[pp * WP + ww] = ldg_stream(&base[(size_t)ww * N + pp]);
-    }
-    for (int idx = tid; idx < (N + 1) * W; idx += NT) {
-        const int ww = idx / (N + 1), k = idx % (N + 1), ky = ky0 + ww;
-        gs[ww * GROW + k] = __ldg(&Ghat[((size_t)kz * (ny + 1) + min(ky, 2 * ny - ky)) * d.gpitch + k]);
+    // Every global load of the CTA is issued before the first shared-memory store: the tile (N W / NT = 8 x 16 bytes per
+    // thread) and the W Green's rows (row ww: entries tid + j NT, the Nyquist entry by thread ww).  Written as load-store
+    // loops the compiler kept one load in flight per thread, and with one CTA per SM the nine round trips to L2 / HBM of
+    // the Green's rows alone took 6 of the 16 us a tile spent on the SM (ncu r3: the STS behind the load held the samples).
+    {
+        constexpr int TIT = N * W / NT, KPR = N / NT;
+        const double *grow0 = Ghat + (size_t)kz * (ny + 1) * d.gpitch;
+        cplx t[TIT];
+        double g[W][KPR], gn = 0.0;
+#pragma unroll
+        for (int it = 0; it < TIT; ++it) t[it] = ldg_stream(&base[tid + it * NT]);
+#pragma unroll
+        for (int ww = 0; ww < W; ++ww) {
+            const int ky = ky0 + ww;
+            const double *row = grow0 + (size_t)min(ky, 2 * ny - ky) * d.gpitch;
+#pragma unroll
+            for (int j = 0; j < KPR; ++j) g[ww][j] = __ldg(&row[tid + j * NT]);
+        }
+        if (tid < W) {
+            const int ky = ky0 + tid;
+            gn = __ldg(&grow0[(size_t)min(ky, 2 * ny - ky) * d.gpitch + N]);
+        }
+#pragma unroll
+        for (int it = 0; it < TIT; ++it) {
+            const int idx = tid + it * NT, ww = idx / N, pp = idx % N;
+            s[pp * WP + ww] = t[it];
+        }
+#pragma unroll
+        for (int ww = 0; ww < W; ++ww)
+#pragma unroll
+            for (int j = 0; j < KPR; ++j) gs[ww * GROW + P3BigGeom<L>::gpos(tid + j * NT)] = g[ww][j];
+        if (tid < W) gs[tid * GROW + P3BigGeom<L>::gpos(N)] = gn;
     }
     __syncthreads();
     cplx v[16];
@@ -189,17 +227,23 @@ p3_x_conv_big(cplx *__restrict__ B, const double *__restrict__ Ghat, MeshDims d,
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const int kx = big_freq_of<L>(16 * u + i);
-        v[i] = cscale(v[i], gs[w * GROW + min(kx, L - kx)]);
+        v[i] = cscale(v[i], gs[w * GROW + P3BigGeom<L>::gpos(min(kx, L - kx))]);
     }
     St::template bfly3<+1>(v);
     St::put3(s, v, u, w);
     __syncthreads();
-    St::template stage2<+1>(s, tw, u, w);
+    // The inverse stages read the same twiddle-table entries as the forward ones (tw[u q], tw[16 j q]).  Seen through the
+    // same `u`, the compiler keeps all 2 x 15 of them in registers from the forward half on (read-only loads are merged) and
+    // spills 270 bytes per thread to make room: at 512 x 512 x 256 that was 9 GB of local-memory traffic through L2 per
+    // launch and a 4.2 ms kernel.  An opaque copy of u makes the inverse half reload them.
+    int ui = u;
+    asm volatile("" : "+r"(ui));
+    St::template stage2<+1>(s, tw, ui, w);
     __syncthreads();
-    St::get1(s, v, u, w);
-    St::inv1(v, tw, u);
+    St::get1(s, v, ui, w);
+    St::inv1(v, tw, ui);
     __syncthreads();                                      // all stage-1 reads done before the cropped result is written
-    St::put1(s, v, u, w, 8);
+    St::put1(s, v, ui, w, 8);
     __syncthreads();
     if (PDL) pdl_trigger();
 #pragma unroll 4

@@ -414,7 +414,7 @@ static void launch_big(const dks_poisson_plan::Step &s, const dks_poisson_plan *
     switch (s.pass) {
     case 1: launch_pdl(p->pdl, p1_z_r2c_big<L, false>, p1_z_r2c_big<L, true>, dim3(d.nx / (2 * G::W), d.ny, nb), dim3(G::THREADS), G::SMEM, st, rho, p->A, d, p->tw[2]); break;
     case 2: launch_pdl(p->pdl, p2_y_fwd_big<L, false>, p2_y_fwd_big<L, true>, dim3(d.nx / G::W, s.planes * nb), dim3(G::THREADS), G::SMEM, st, p->A, p->B, d, s.kz0, p->tw[1]); break;
-    case 3: launch_pdl(p->pdl, p3_x_conv_big<L, false>, p3_x_conv_big<L, true>, dim3((unsigned)((size_t)s.planes * nb * 2 * d.ny / G::W)), dim3(G::THREADS), P3BigGeom<L>::SMEM, st, p->B, p->G, d, s.kz0, p->tw[0]); break;
+    case 3: launch_pdl(p->pdl, p3_x_conv_big<L, false>, p3_x_conv_big<L, true>, dim3((unsigned)((size_t)s.planes * nb * 2 * d.ny / P3BigGeom<L>::W)), dim3(P3BigGeom<L>::THREADS), P3BigGeom<L>::SMEM, st, p->B, p->G, d, s.kz0, p->tw[0]); break;
     case 4: launch_pdl(p->pdl, p4_y_inv_big<L, false>, p4_y_inv_big<L, true>, dim3(d.nx / G::W, s.planes * nb), dim3(G::THREADS), G::SMEM, st, p->B, p->A, d, s.kz0, p->tw[1]); break;
     case 5: launch_pdl(p->pdl, p5_z_c2r_big<L, false>, p5_z_c2r_big<L, true>, dim3(d.nx / (2 * G::W), d.ny, nb), dim3(G::THREADS), G::SMEM, st, p->A, phi, d, p->tw[2]); break;
     }

@@ -146,6 +146,51 @@ def test_paper_table1_largest_shape_sampled(torch_cuda, dks, oracle, workloads):
     assert np.max(np.abs(g - direct) / np.abs(direct)) <= 1e-11
 
 
+@pytest.mark.slow
+def test_paper_table1_largest_shape_1000_nodes_and_library_fft(torch_cuda, dks, oracle, workloads):
+    # The only large workload of p2_y_fwd_big / p3_x_conv_big / p4_y_inv_big.  The oracle's doubled-grid arrays
+    # would need 2 x 8.6 GB of host memory here, so: (i) Eq. (2) summed directly by the oracle at 1009 sampled nodes (about 40 s
+    # of host time), and (ii) EVERY node against the same convolution through torch.fft (cuFFT) -- a third opinion, not the oracle,
+    # which ties the unsampled nodes to the sampled ones: a wrong row, tile or plane anywhere fails (ii), a common error (i).
+    torch = torch_cuda
+    n, h = (512, 512, 256), (1e-4, 1e-4, 2e-4)
+    (nx, ny, nz), (hx, hy, hz) = n, h
+    rho = workloads.random_rho(n, seed=98, signed=False)
+    d_rho = torch.from_numpy(rho).cuda()
+    plan = dks.PoissonPlan(n, h, host_staging=False)
+    try:
+        got_d = plan.solve(d_rho)
+        torch.cuda.synchronize()
+    finally:
+        plan.close()
+    got = got_d.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    nodes = workloads.sample_nodes(n, 8, count=1000)
+    direct = oracle.direct_sum_nodes(rho, n, h, nodes, precision="ld")
+    g = got[nodes[:, 2], nodes[:, 1], nodes[:, 0]]
+    assert np.max(np.abs(g - direct)) <= MAX_ABS_TOL * np.max(np.abs(got))
+    assert np.linalg.norm(g - direct) <= REL_L2_TOL * np.linalg.norm(direct)
+
+    def mirrored(m, hh):
+        i = torch.arange(2 * m, device="cuda", dtype=torch.float64)
+        return torch.minimum(i, 2 * m - i) * hh
+
+    r = torch.sqrt(mirrored(nz, hz)[:, None, None] ** 2 + mirrored(ny, hy)[None, :, None] ** 2 + mirrored(nx, hx)[None, None, :] ** 2)
+    r[0, 0, 0] = 0.5 * min(hx, hy, hz)
+    ghat = torch.fft.rfftn(1.0 / (4.0 * np.pi * 8.8541878128e-12 * r))
+    del r
+    shape = (2 * nz, 2 * ny, 2 * nx)
+    spec = torch.fft.rfftn(d_rho, s=shape)
+    spec *= ghat
+    del ghat
+    ref = torch.fft.irfftn(spec, s=shape)[:nz, :ny, :nx] * (hx * hy * hz)
+    del spec
+    assert float(torch.linalg.norm((got_d - ref).flatten()) / torch.linalg.norm(ref.flatten())) <= REL_L2_TOL
+    assert float((got_d - ref).abs().max()) <= MAX_ABS_TOL * float(ref.abs().max())
+    del ref, got_d
+    torch.cuda.empty_cache()
+
+
 def test_full_size_agreement_with_a_library_fft_on_the_gpu(torch_cuda, dks, workloads):
     # A third opinion at a size the long-double oracle needs minutes for: the same convolution through torch.fft (cuFFT) on the doubled
     # grid of config 3 (the library special case of pin P12, run on the GPU).  Not the oracle: an independent FFT, same readings A1-A5.
